@@ -1,0 +1,10 @@
+"""CPU oracle for the log-polar thin-disk potential -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It never imports paper_2409_02294_b200.
+"""
+from .polar_oracle import (  # noqa: F401
+    build, grid, potential_o0, potential_o0_targets, potential_o1, potential_o1_rings,
+    num_threads,
+)
+from .definition_numpy import potential_definition_numpy  # noqa: F401
