@@ -1,0 +1,158 @@
+/*
+ * polargrav.h -- C ABI of libpolargrav.so (B200 / sm_100a only).
+ *
+ * Gravitational potential of a razor-thin disk on a log-polar grid,
+ *
+ *     Phi_ij = -G * sum_{i'j'} Sigma_{i'j'} dA_{i'} / sqrt(d2(i,j;i',j')),      G = 1,
+ *     d2     = (r_i - r_i')^2 + 4 r_i r_i' sin^2((phi_j - phi_j')/2) + eps^2 h_i h_i',
+ *
+ * evaluated as a zero-padded FFT convolution on the GPU ("the convolution method for
+ * solving potential fields"; "FFT operations" are the GPU-resident work,
+ * PAPER.md:19).  PAPER.md prints no formula; the sum is BASELINE.json north_star's and
+ * every convention is a reading listed in DESIGN.md section 3 (A1..A8):
+ *
+ *     edges   re_i = r_in (r_out/r_in)^(i/n_r);  centres r_i = sqrt(re_i re_{i+1}) = r_in exp((i+1/2) du)
+ *     phi_j   = (j+1/2) dphi,  dphi = 2 pi / n_phi,  du = ln(r_out/r_in)/n_r
+ *     dA_i    = (re_{i+1}^2 - re_i^2) dphi / 2 = r_i^2 sinh(du) dphi;   h_i = sqrt(dA_i)
+ *     the self term (i'=i, j'=j) is included: it contributes -Sigma_ij h_i / eps.
+ *
+ * The seam is a C ABI on purpose: the paper's own conclusion is that a C binding is the
+ * robust boundary between tool-chains, with addresses handed across once and no hidden
+ * copies (App. A :397-400), and that the CUDA side should own the pinned
+ * host memory (Fig. 4 :202).
+ *
+ * Conventions for every call
+ *   - Arrays are C order [batch][n_r][n_phi], phi fastest, contiguous, IEEE fp64.
+ *   - No C++ types, no exceptions, never abort(): every call returns a pg_status;
+ *     pg_last_error() gives the text of the last failure on that solver.
+ *   - There is NO CPU fallback and no alternative backend: without a CUDA device of
+ *     compute capability 10.x pg_create* fails with PG_ERR_UNSUPPORTED / PG_ERR_CUDA.
+ *   - One solver per host thread at a time; distinct solvers are independent.
+ */
+#ifndef POLARGRAV_H
+#define POLARGRAV_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pg_solver pg_solver; /* opaque */
+
+typedef enum {
+    PG_OK = 0,
+    PG_ERR_INVALID_ARG = -1, /* null pointer, r_in<=0, r_out<=r_in, eps<=0, batch out of range */
+    PG_ERR_UNSUPPORTED = -2, /* n_r/n_phi not a power of two in [PG_MIN_N, PG_MAX_N], device not sm_100 */
+    PG_ERR_CUDA = -3,        /* a CUDA call failed; text in pg_last_error */
+    PG_ERR_NOMEM = -4,       /* host or device allocation failed */
+    PG_ERR_STATE = -5        /* pg_potential* before any pg_set_density */
+} pg_status;
+
+/* Where a caller-owned buffer lives. */
+typedef enum {
+    PG_MEM_HOST = 0,        /* pageable host memory: staged through the solver's pinned buffer */
+    PG_MEM_HOST_PINNED = 1, /* page-locked host memory (e.g. from pg_host_alloc): async copy, no staging */
+    PG_MEM_DEVICE = 2       /* device memory on the solver's device */
+} pg_memspace;
+
+#define PG_MIN_N 32
+#define PG_MAX_N 2048
+
+/*
+ * pg_create / pg_create_ex -- build a solver for one grid (north_star: pg_create(grid: N_r, N_phi,
+ * r_in, r_out, eps)).  One-time work (row a1 of DESIGN.md): Green's kernel
+ *     K(k,l) = [4 sinh^2(k du/2) + 4 sin^2(l dphi/2) + eta^2]^(-1/2),  eta^2 = eps^2 sinh(du) dphi,
+ * on the lags k in (-n_r, n_r), l in [0, n_phi), its 2-D FFT on the 2 n_r x n_phi padded lag grid
+ * (real, because K is even in both lags), with -G sinh(du) dphi and the FFT normalisation folded in.
+ *
+ *   out        receives the solver; *out is set to NULL on failure.
+ *   n_r,n_phi  powers of two in [PG_MIN_N, PG_MAX_N].
+ *   r_in,r_out inner / outer EDGE of the grid, 0 < r_in < r_out.
+ *   eps        dimensionless softening in units of the local cell size h = sqrt(dA), > 0.
+ *   max_batch  largest `batch` later calls may pass (>= 1); workspace scales with it.
+ *   device     CUDA device ordinal, or -1 for the current device.
+ *   cuda_stream a cudaStream_t (borrowed, may be NULL = the legacy default stream).  All work
+ *              of this solver is enqueued on it.
+ * Ownership: the solver owns the spectrum, tables, workspace and pinned staging buffers.
+ */
+pg_status pg_create(pg_solver **out, int n_r, int n_phi, double r_in, double r_out, double eps);
+pg_status pg_create_ex(pg_solver **out, int n_r, int n_phi, double r_in, double r_out, double eps,
+                       int max_batch, int device, void *cuda_stream);
+
+/*
+ * pg_set_density -- hand the surface density Sigma[batch][n_r][n_phi] to the solver.
+ *   PG_MEM_DEVICE      : BORROWED, no copy.  Must stay valid and unmodified until the work of the
+ *                        following pg_potential* call has completed on the stream.
+ *   PG_MEM_HOST_PINNED : cudaMemcpyAsync to an owned device buffer; returns after enqueue; the
+ *                        caller must not modify `sigma` until the stream has passed the copy.
+ *   PG_MEM_HOST        : memcpy into the owned pinned staging buffer, then cudaMemcpyAsync; returns
+ *                        once `sigma` may be reused (row a6; pinned staging per PAPER.md:97-101,:119).
+ * 1 <= batch <= max_batch.  NaN/Inf/negative values are not checked and propagate (linearity).
+ */
+pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspace where);
+
+/*
+ * pg_potential -- FFT-convolution solve (rows a2-a4): writes Phi[batch][n_r][n_phi] for the density
+ * last set; `batch` must equal that call's batch.
+ *   PG_MEM_DEVICE / PG_MEM_HOST_PINNED : returns after enqueue (use pg_synchronize or sync the stream).
+ *   PG_MEM_HOST                        : blocks until `phi` is filled.
+ * For host memspaces with batch > 1 the copies of one field overlap the solves of its neighbours
+ * (separate copy stream + events).  `phi` may not alias the density.
+ */
+pg_status pg_potential(pg_solver *s, double *phi, int batch, pg_memspace where);
+
+/*
+ * pg_potential_direct -- tiled all-pairs direct summation on the GPU (row a5), evaluated from the
+ * coordinates, used as an on-device cross-check of pg_potential.  O((n_r n_phi)^2): seconds at
+ * 512^2, not meant for production.  Same argument rules as pg_potential.  NOT a fallback: nothing
+ * in the library calls it.
+ * pg_potential_direct_rings -- the same for target rings [ring0, ring0+n_rings) of field 0 only;
+ * `phi` receives [n_rings][n_phi].
+ */
+pg_status pg_potential_direct(pg_solver *s, double *phi, int batch, pg_memspace where);
+pg_status pg_potential_direct_rings(pg_solver *s, double *phi, int ring0, int n_rings, pg_memspace where);
+
+/* pg_destroy -- frees everything the solver owns. pg_destroy(NULL) is a no-op returning PG_OK. */
+pg_status pg_destroy(pg_solver *s);
+
+/* ---------------------------------------------------------------- helpers */
+
+/* Grid tables (host pointers, any may be NULL): r[n_r] cell-centre radii, phi[n_phi] cell-centre
+ * azimuths, cell_area[n_r] exact sector areas.  Callers never need to recompute conventions. */
+pg_status pg_grid(const pg_solver *s, double *r, double *phi, double *cell_area);
+
+/* Replace the (borrowed) stream; synchronises the old one first. */
+pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
+/* Block until all work enqueued by this solver has completed. */
+pg_status pg_synchronize(pg_solver *s);
+
+/* Page-locked host memory owned by the CUDA side (Fig. 4).  Needs a CUDA device. */
+pg_status pg_host_alloc(void **p, size_t bytes);
+pg_status pg_host_free(void *p);
+
+/* Per-kernel device timing.  When enabled, CUDA events are recorded around each kernel of
+ * pg_potential on the solver's stream; pg_kernel_times returns the accumulated milliseconds and
+ * launch counts since the last pg_profile(s, 1) call (it synchronises the stream).
+ *   index 0: a2 row forward (pre-weight + phi R2C)   1: a3+a4r column pass (FFT, x K^, IFFT, crop)
+ *   index 2: a4 row inverse (phi C2R + post-scale)                                              */
+#define PG_NUM_KERNELS 3
+pg_status pg_profile(pg_solver *s, int enable);
+pg_status pg_kernel_times(pg_solver *s, double ms[PG_NUM_KERNELS], long launches[PG_NUM_KERNELS]);
+
+/* Number of kernels this library has launched on behalf of `s` since creation. */
+long pg_launch_count(const pg_solver *s);
+
+/* Algorithmic HBM bytes of one pg_potential call of `batch` fields, and of
+ * kernel `index` alone (same indices as pg_kernel_times). */
+double pg_algorithmic_bytes(const pg_solver *s, int batch);
+double pg_kernel_algorithmic_bytes(const pg_solver *s, int index, int batch);
+
+const char *pg_status_string(pg_status st);
+const char *pg_last_error(const pg_solver *s); /* s may be NULL: last error of a failed pg_create* */
+const char *pg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POLARGRAV_H */

@@ -1,0 +1,250 @@
+"""Thin ctypes binding over libpolargrav.so -- argument marshalling only.
+
+Same names as include/polargrav.h.  Every step of the numerical path runs in the CUDA
+kernels; nothing here computes.  If the library is missing this module raises -- there
+is no CPU fallback.  PyTorch (optional) is used by callers only for device memory and
+streams: pass `tensor.data_ptr()` / `stream.cuda_stream`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpolargrav.so")
+
+PG_OK = 0
+PG_ERR_INVALID_ARG, PG_ERR_UNSUPPORTED, PG_ERR_CUDA, PG_ERR_NOMEM, PG_ERR_STATE = -1, -2, -3, -4, -5
+PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
+PG_NUM_KERNELS = 3
+KERNEL_NAMES = ("rows_fwd(a2)", "cols(a3+a4r)", "rows_inv(a4phi)")
+
+# every symbol include/polargrav.h declares
+EXPORTS = (
+    "pg_create", "pg_create_ex", "pg_set_density", "pg_potential", "pg_potential_direct",
+    "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_synchronize",
+    "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
+    "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
+    "pg_version",
+)
+
+_lib = None
+
+
+class PolargravError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(f"{status_string(status)} ({status}): {message}")
+        self.status = status
+
+
+def lib():
+    """Loads libpolargrav.so (once).  Raises if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} not found: build it with `python -m paper_2409_02294_b200.build` "
+                "(nvcc, sm_100a).  There is no CPU fallback.")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i, d, l = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_long
+        L.pg_create.argtypes = [ctypes.POINTER(vp), i, i, d, d, d]
+        L.pg_create_ex.argtypes = [ctypes.POINTER(vp), i, i, d, d, d, i, i, vp]
+        L.pg_set_density.argtypes = [vp, vp, i, i]
+        L.pg_potential.argtypes = [vp, vp, i, i]
+        L.pg_potential_direct.argtypes = [vp, vp, i, i]
+        L.pg_potential_direct_rings.argtypes = [vp, vp, i, i, i]
+        L.pg_destroy.argtypes = [vp]
+        L.pg_grid.argtypes = [vp, vp, vp, vp]
+        L.pg_set_stream.argtypes = [vp, vp]
+        L.pg_synchronize.argtypes = [vp]
+        L.pg_host_alloc.argtypes = [ctypes.POINTER(vp), ctypes.c_size_t]
+        L.pg_host_free.argtypes = [vp]
+        L.pg_profile.argtypes = [vp, i]
+        L.pg_kernel_times.argtypes = [vp, ctypes.POINTER(d), ctypes.POINTER(l)]
+        for name in EXPORTS:
+            getattr(L, name).restype = i
+        L.pg_launch_count.argtypes = [vp]; L.pg_launch_count.restype = l
+        L.pg_algorithmic_bytes.argtypes = [vp, i]; L.pg_algorithmic_bytes.restype = d
+        L.pg_kernel_algorithmic_bytes.argtypes = [vp, i, i]; L.pg_kernel_algorithmic_bytes.restype = d
+        L.pg_status_string.argtypes = [i]; L.pg_status_string.restype = ctypes.c_char_p
+        L.pg_last_error.argtypes = [vp]; L.pg_last_error.restype = ctypes.c_char_p
+        L.pg_version.argtypes = []; L.pg_version.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def status_string(st: int) -> str:
+    return lib().pg_status_string(int(st)).decode()
+
+
+def last_error(handle=None) -> str:
+    return lib().pg_last_error(handle).decode()
+
+
+def version() -> str:
+    return lib().pg_version().decode()
+
+
+def _check(st, handle=None):
+    if st != PG_OK:
+        raise PolargravError(st, last_error(handle))
+
+
+def _ptr(x):
+    """Address of a numpy array / int address / object with data_ptr() (torch tensor)."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        if x.dtype != np.float64 or not x.flags.c_contiguous:
+            raise TypeError("arrays must be C-contiguous float64")
+        return x.ctypes.data
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    return int(x)
+
+
+# ------------------------------------------------------------------ the C ABI, same names
+def pg_create(n_r, n_phi, r_in, r_out, eps):
+    h = ctypes.c_void_p()
+    st = lib().pg_create(ctypes.byref(h), n_r, n_phi, r_in, r_out, eps)
+    _check(st)
+    return h
+
+
+def pg_create_ex(n_r, n_phi, r_in, r_out, eps, max_batch=1, device=-1, cuda_stream=None):
+    h = ctypes.c_void_p()
+    st = lib().pg_create_ex(ctypes.byref(h), n_r, n_phi, r_in, r_out, eps, max_batch, device,
+                            ctypes.c_void_p(cuda_stream) if cuda_stream else None)
+    _check(st)
+    return h
+
+
+def pg_set_density(h, sigma, batch, where):
+    _check(lib().pg_set_density(h, _ptr(sigma), batch, where), h)
+
+
+def pg_potential(h, phi, batch, where):
+    _check(lib().pg_potential(h, _ptr(phi), batch, where), h)
+
+
+def pg_potential_direct(h, phi, batch, where):
+    _check(lib().pg_potential_direct(h, _ptr(phi), batch, where), h)
+
+
+def pg_potential_direct_rings(h, phi, ring0, n_rings, where):
+    _check(lib().pg_potential_direct_rings(h, _ptr(phi), ring0, n_rings, where), h)
+
+
+def pg_destroy(h):
+    _check(lib().pg_destroy(h))
+
+
+def pg_grid(h, n_r, n_phi):
+    r, phi, area = np.empty(n_r), np.empty(n_phi), np.empty(n_r)
+    _check(lib().pg_grid(h, r.ctypes.data, phi.ctypes.data, area.ctypes.data), h)
+    return r, phi, area
+
+
+def pg_set_stream(h, cuda_stream):
+    _check(lib().pg_set_stream(h, ctypes.c_void_p(cuda_stream) if cuda_stream else None), h)
+
+
+def pg_synchronize(h):
+    _check(lib().pg_synchronize(h), h)
+
+
+def pg_host_alloc(nbytes):
+    p = ctypes.c_void_p()
+    _check(lib().pg_host_alloc(ctypes.byref(p), nbytes))
+    return p.value
+
+
+def pg_host_free(p):
+    _check(lib().pg_host_free(ctypes.c_void_p(p)))
+
+
+def pg_profile(h, enable):
+    _check(lib().pg_profile(h, int(bool(enable))), h)
+
+
+def pg_kernel_times(h):
+    ms = (ctypes.c_double * PG_NUM_KERNELS)()
+    n = (ctypes.c_long * PG_NUM_KERNELS)()
+    _check(lib().pg_kernel_times(h, ms, n), h)
+    return list(ms), list(n)
+
+
+def pg_launch_count(h):
+    return int(lib().pg_launch_count(h))
+
+
+def pg_algorithmic_bytes(h, batch=1):
+    return float(lib().pg_algorithmic_bytes(h, batch))
+
+
+def pg_kernel_algorithmic_bytes(h, index, batch=1):
+    return float(lib().pg_kernel_algorithmic_bytes(h, index, batch))
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class PinnedArray:
+    """float64 numpy view over page-locked memory owned by the CUDA side (pg_host_alloc)."""
+
+    def __init__(self, shape):
+        self.shape = tuple(shape)
+        n = int(np.prod(self.shape))
+        self.ptr = pg_host_alloc(n * 8)
+        buf = (ctypes.c_double * n).from_address(self.ptr)
+        self.array = np.frombuffer(buf, dtype=np.float64).reshape(self.shape)
+
+    def free(self):
+        if self.ptr:
+            self.array = None
+            pg_host_free(self.ptr)
+            self.ptr = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Solver:
+    """RAII wrapper; methods marshal arguments and call the C ABI, nothing else."""
+
+    def __init__(self, n_r, n_phi, r_in, r_out, eps, max_batch=1, device=-1, cuda_stream=None):
+        self.n_r, self.n_phi, self.max_batch = n_r, n_phi, max_batch
+        self.h = pg_create_ex(n_r, n_phi, r_in, r_out, eps, max_batch, device, cuda_stream)
+
+    def grid(self):
+        return pg_grid(self.h, self.n_r, self.n_phi)
+
+    def potential_host(self, sigma: np.ndarray, direct: bool = False) -> np.ndarray:
+        """Host numpy in, host numpy out (pageable path, PG_MEM_HOST)."""
+        s = np.ascontiguousarray(sigma, dtype=np.float64)
+        batch = 1 if s.ndim == 2 else s.shape[0]
+        if s.shape[-2:] != (self.n_r, self.n_phi):
+            raise ValueError("sigma has the wrong shape")
+        out = np.empty_like(s)
+        pg_set_density(self.h, s, batch, PG_MEM_HOST)
+        (pg_potential_direct if direct else pg_potential)(self.h, out, batch, PG_MEM_HOST)
+        return out
+
+    def close(self):
+        if self.h is not None:
+            pg_destroy(self.h)
+            self.h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

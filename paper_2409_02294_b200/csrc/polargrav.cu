@@ -1,0 +1,773 @@
+// polargrav.cu -- C ABI (include/polargrav.h) and host-side runtime of libpolargrav.so.
+//
+// Host logic only: argument checks, table construction (long double), buffer ownership,
+// stream/event plumbing for the pinned staging pipeline (row a6), kernel dispatch by grid size.
+// Every step of the numerical path runs in the kernels of kernels.cuh.  There is no CPU
+// fallback: without an sm_100 device pg_create* fails.
+#include "../../include/polargrav.h"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using pgk::cplx;
+
+namespace {
+
+constexpr int kMaxProfiledCalls = 2048;
+
+thread_local char g_create_error[512] = "";
+
+struct Events4 { cudaEvent_t e[4]; };
+
+}  // namespace
+
+struct pg_solver {
+    int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
+    double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
+    int m_h = 0;       // n_phi/2 + 1 azimuthal modes
+    int m_c = 0;       // padded to a multiple of cols_per_cta(n_r)
+    size_t field = 0;  // n_r * n_phi
+
+    cudaStream_t stream = nullptr;             // borrowed
+    cudaStream_t h2d = nullptr, d2h = nullptr; // owned copy streams
+    std::vector<cudaEvent_t> ev_in, ev_solved, ev_out;
+    cudaEvent_t ev_main = nullptr;
+    std::vector<char> in_pending;
+
+    // device memory (owned)
+    cplx *d_W = nullptr;          // [max_batch][m_c][n_r]
+    double *d_khat = nullptr;     // [m_c][2][n_r]
+    cplx *d_tw_row = nullptr, *d_rtw = nullptr, *d_itw = nullptr;
+    cplx *d_tw_col = nullptr, *d_mod = nullptr;
+    double *d_rs_in = nullptr, *d_rs_out = nullptr;
+    double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
+    double *d_sigma_own = nullptr, *d_phi_own = nullptr;   // [max_batch][n_r][n_phi], lazily allocated
+    // pinned host staging (owned, lazily allocated)
+    double *h_in = nullptr, *h_out = nullptr;
+
+    // current density
+    const double *d_sigma = nullptr;
+    int cur_batch = 0;
+    bool sigma_from_host = false;
+
+    // host tables
+    std::vector<double> r, phi, dA;
+
+    // profiling
+    bool profile = false;
+    std::vector<Events4> prof_pool;
+    int prof_used = 0;
+    double prof_ms[PG_NUM_KERNELS] = {0, 0, 0};
+    long prof_n[PG_NUM_KERNELS] = {0, 0, 0};
+    long launches = 0;
+
+    char err[512] = "";
+};
+
+namespace {
+
+void set_err(pg_solver *s, const char *fmt, ...)
+{
+    char *dst = s ? s->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+}
+
+#define PG_CUDA(s, call)                                                                       \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            set_err((s), "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__,     \
+                    __LINE__);                                                                 \
+            return e_ == cudaErrorMemoryAllocation ? PG_ERR_NOMEM : PG_ERR_CUDA;               \
+        }                                                                                      \
+    } while (0)
+
+bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// ------------------------------------------------------------------ tables
+const long double kPiL = 3.141592653589793238462643383279502884L;
+
+cplx unit(long double turns)   // exp(-2 pi i turns)
+{
+    const long double a = 2.0L * kPiL * turns;
+    return make_double2((double)cosl(a), (double)(-sinl(a)));
+}
+
+// [tw0 | tw1] of pgk::Plan for a length-L transform (see fft.cuh)
+std::vector<cplx> fft_tables(int L)
+{
+    const int n16 = (L >= 256) ? 2 : 1;
+    const int R1 = L / (n16 == 2 ? 256 : 16);
+    const int T2 = L / R1, T3 = T2 / 16;
+    std::vector<cplx> t;
+    if (R1 > 1)
+        for (int k = 0; k < R1; ++k)
+            for (int b = 0; b < T2; ++b) t.push_back(unit((long double)b * k / L));
+    if (n16 == 2)
+        for (int k = 0; k < 16; ++k)
+            for (int q = 0; q < T3; ++q) t.push_back(unit((long double)q * k / T2));
+    if (t.empty()) t.push_back(make_double2(1.0, 0.0));
+    return t;
+}
+
+template <class T>
+pg_status upload(pg_solver *s, T **dst, const std::vector<T> &src)
+{
+    PG_CUDA(s, cudaMalloc((void **)dst, src.size() * sizeof(T)));
+    PG_CUDA(s, cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return PG_OK;
+}
+
+// ------------------------------------------------------------------ kernel dispatch
+template <int NPHI>
+pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rscale, int n_rows,
+                          int batch, long sigma_stride, long w_stride, cudaStream_t st)
+{
+    typedef pgk::RowShape<NPHI> S;
+    dim3 grid(n_rows / S::ROWS, batch);
+    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, W, s->d_tw_row, s->d_rtw, rscale, n_rows,
+                                                                 sigma_stride, w_stride);
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+template <int NPHI>
+pg_status launch_rows_inv(pg_solver *s, const cplx *W, double *phi, int batch, long w_stride, long phi_stride,
+                          cudaStream_t st)
+{
+    typedef pgk::RowShape<NPHI> S;
+    dim3 grid(s->n_r / S::ROWS, batch);
+    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(W, phi, s->d_tw_row, s->d_itw, s->d_rs_out, s->n_r,
+                                                                 w_stride, phi_stride);
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+template <int NR>
+pg_status launch_cols(pg_solver *s, cplx *W, int batch, long w_stride, cudaStream_t st)
+{
+    typedef pgk::ColShape<NR> S;
+    dim3 grid(s->m_c / S::C, batch);
+    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(W, s->d_khat, s->d_tw_col, s->d_mod, w_stride);
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+template <int NR>
+pg_status launch_khat_cols(pg_solver *s, const cplx *Wk, double scale, cudaStream_t st)
+{
+    typedef pgk::ColShape<NR> S;
+    dim3 grid(s->m_c / S::C, 1);
+    pgk::khat_cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Wk, s->d_khat, s->d_tw_col, s->d_mod, scale, s->m_h);
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+// opt in to > 48 KiB of dynamic shared memory, once per solver (the attribute is per device)
+template <int NPHI>
+pg_status prepare_rows(pg_solver *s)
+{
+    typedef pgk::RowShape<NPHI> S;
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::rows_fwd_kernel<NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)S::SMEM));
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::rows_inv_kernel<NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)S::SMEM));
+    return PG_OK;
+}
+template <int NR>
+pg_status prepare_cols(pg_solver *s)
+{
+    typedef pgk::ColShape<NR> S;
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)S::SMEM));
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::khat_cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)S::SMEM));
+    return PG_OK;
+}
+
+#define PG_DISPATCH(n, CALL)                                                   \
+    switch (n) {                                                               \
+        case 32: return CALL(32);                                              \
+        case 64: return CALL(64);                                              \
+        case 128: return CALL(128);                                            \
+        case 256: return CALL(256);                                            \
+        case 512: return CALL(512);                                            \
+        case 1024: return CALL(1024);                                          \
+        case 2048: return CALL(2048);                                          \
+        default: set_err(s, "unsupported size %d", (n)); return PG_ERR_UNSUPPORTED; \
+    }
+
+pg_status rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rscale, int n_rows, int batch,
+                   long sigma_stride, long w_stride, cudaStream_t st)
+{
+#define CALL(N) launch_rows_fwd<N>(s, sigma, W, rscale, n_rows, batch, sigma_stride, w_stride, st)
+    PG_DISPATCH(s->n_phi, CALL)
+#undef CALL
+}
+pg_status rows_inv(pg_solver *s, const cplx *W, double *phi, int batch, long w_stride, long phi_stride,
+                   cudaStream_t st)
+{
+#define CALL(N) launch_rows_inv<N>(s, W, phi, batch, w_stride, phi_stride, st)
+    PG_DISPATCH(s->n_phi, CALL)
+#undef CALL
+}
+pg_status cols(pg_solver *s, cplx *W, int batch, long w_stride, cudaStream_t st)
+{
+#define CALL(N) launch_cols<N>(s, W, batch, w_stride, st)
+    PG_DISPATCH(s->n_r, CALL)
+#undef CALL
+}
+pg_status prepare_kernels_rows(pg_solver *s)
+{
+#define CALL(N) prepare_rows<N>(s)
+    PG_DISPATCH(s->n_phi, CALL)
+#undef CALL
+}
+pg_status prepare_kernels_cols(pg_solver *s)
+{
+#define CALL(N) prepare_cols<N>(s)
+    PG_DISPATCH(s->n_r, CALL)
+#undef CALL
+}
+pg_status khat_cols(pg_solver *s, const cplx *Wk, double scale, cudaStream_t st)
+{
+#define CALL(N) launch_khat_cols<N>(s, Wk, scale, st)
+    PG_DISPATCH(s->n_r, CALL)
+#undef CALL
+}
+
+// ------------------------------------------------------------------ one-time spectrum of the Green's kernel (a1)
+pg_status build_khat(pg_solver *s)
+{
+    const int n_r = s->n_r, n_phi = s->n_phi;
+    double *d_kpad = nullptr;
+    cplx *d_wk = nullptr;
+    const size_t kpad_n = (size_t)2 * n_r * n_phi;
+    const size_t wk_n = (size_t)s->m_c * 2 * n_r;
+    PG_CUDA(s, cudaMalloc((void **)&d_kpad, kpad_n * sizeof(double)));
+    cudaError_t e = cudaMalloc((void **)&d_wk, wk_n * sizeof(cplx));
+    if (e != cudaSuccess) {
+        cudaFree(d_kpad);
+        set_err(s, "cudaMalloc(kernel workspace) failed: %s", cudaGetErrorString(e));
+        return PG_ERR_NOMEM;
+    }
+    pg_status st = PG_OK;
+    do {
+        if (cudaMemsetAsync(d_wk, 0, wk_n * sizeof(cplx), s->stream) != cudaSuccess) { st = PG_ERR_CUDA; break; }
+        const double eta2 = s->eps * s->eps * std::sinh(s->du) * s->dphi;
+        const int threads = 256;
+        const long blocks = (long)((kpad_n + threads - 1) / threads);
+        pgk::green_fill_kernel<<<(unsigned)blocks, threads, 0, s->stream>>>(d_kpad, n_r, n_phi, s->du, eta2);
+        s->launches++;
+        if (cudaGetLastError() != cudaSuccess) { st = PG_ERR_CUDA; break; }
+        // phi transform of the 2 n_r lag rows (no radial weight), transposed into Wk[m][2 n_r]
+        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream);
+        if (st != PG_OK) break;
+        // -G sinh(du) dphi (cell area / r^2), and the normalisation of the unnormalised transforms:
+        // 1/(2 n_r) for the padded radial pair, 1/n_phi for the azimuthal pair (the rows_inv
+        // pre-processing builds 2 Z, and the packed complex transform has length n_phi/2).
+        const double scale = -std::sinh(s->du) * s->dphi / (2.0 * (double)n_r * (double)n_phi);
+        st = khat_cols(s, d_wk, scale, s->stream);
+        if (st != PG_OK) break;
+        if (cudaStreamSynchronize(s->stream) != cudaSuccess) { st = PG_ERR_CUDA; break; }
+    } while (0);
+    if (st == PG_ERR_CUDA && s->err[0] == 0) set_err(s, "Green's kernel precompute failed: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaFree(d_kpad);
+    cudaFree(d_wk);
+    return st;
+}
+
+pg_status ensure_staging(pg_solver *s, bool need_in, bool need_out)
+{
+    const size_t bytes = s->field * (size_t)s->max_batch * sizeof(double);
+    if (need_in && !s->d_sigma_own) PG_CUDA(s, cudaMalloc((void **)&s->d_sigma_own, bytes));
+    if (need_out && !s->d_phi_own) PG_CUDA(s, cudaMalloc((void **)&s->d_phi_own, bytes));
+    return PG_OK;
+}
+pg_status ensure_pinned(pg_solver *s, bool in, bool out)
+{
+    const size_t bytes = s->field * (size_t)s->max_batch * sizeof(double);
+    if (in && !s->h_in) PG_CUDA(s, cudaHostAlloc((void **)&s->h_in, bytes, cudaHostAllocDefault));
+    if (out && !s->h_out) PG_CUDA(s, cudaHostAlloc((void **)&s->h_out, bytes, cudaHostAllocDefault));
+    return PG_OK;
+}
+
+pg_status drain_profile(pg_solver *s)
+{
+    if (s->prof_used == 0) return PG_OK;
+    PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    for (int c = 0; c < s->prof_used; ++c) {
+        for (int k = 0; k < PG_NUM_KERNELS; ++k) {
+            float ms = 0.f;
+            PG_CUDA(s, cudaEventElapsedTime(&ms, s->prof_pool[c].e[k], s->prof_pool[c].e[k + 1]));
+            s->prof_ms[k] += ms;
+            s->prof_n[k] += 1;
+        }
+    }
+    s->prof_used = 0;
+    return PG_OK;
+}
+
+// the three kernels of one solve of `batch` fields starting at the given pointers
+pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx *d_W, int batch)
+{
+    const long fs = (long)s->field, ws = (long)s->m_c * s->n_r;
+    Events4 *ev = nullptr;
+    if (s->profile) {
+        if (s->prof_used == kMaxProfiledCalls) {
+            pg_status st = drain_profile(s);
+            if (st != PG_OK) return st;
+        }
+        if ((int)s->prof_pool.size() <= s->prof_used) {
+            Events4 q;
+            for (int k = 0; k < 4; ++k) PG_CUDA(s, cudaEventCreate(&q.e[k]));
+            s->prof_pool.push_back(q);
+        }
+        ev = &s->prof_pool[s->prof_used++];
+        PG_CUDA(s, cudaEventRecord(ev->e[0], s->stream));
+    }
+    pg_status st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream);
+    if (st != PG_OK) return st;
+    if (ev) PG_CUDA(s, cudaEventRecord(ev->e[1], s->stream));
+    st = cols(s, d_W, batch, ws, s->stream);
+    if (st != PG_OK) return st;
+    if (ev) PG_CUDA(s, cudaEventRecord(ev->e[2], s->stream));
+    st = rows_inv(s, d_W, d_phi, batch, ws, fs, s->stream);
+    if (st != PG_OK) return st;
+    if (ev) PG_CUDA(s, cudaEventRecord(ev->e[3], s->stream));
+    return PG_OK;
+}
+
+pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int ring0, int n_rings, int batch)
+{
+    const int threads = s->n_phi < 256 ? s->n_phi : 256;
+    const int tpt = s->n_phi / threads;
+    const size_t smem = 2 * (size_t)s->n_phi * sizeof(double);
+    const double eps2 = s->eps * s->eps;
+    dim3 grid(n_rings, batch);
+    const long fs = (long)s->field;
+#define DIRECT(TPT)                                                                                          \
+    pgk::direct_kernel<TPT><<<grid, threads, smem, s->stream>>>(d_sigma, d_phi, s->d_r, s->d_dA, s->d_s2, s->n_r, \
+                                                                 s->n_phi, eps2, ring0, fs, fs)
+    switch (tpt) {
+        case 1: DIRECT(1); break;
+        case 2: DIRECT(2); break;
+        case 4: DIRECT(4); break;
+        case 8: DIRECT(8); break;
+        default: set_err(s, "direct: unsupported n_phi"); return PG_ERR_UNSUPPORTED;
+    }
+#undef DIRECT
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+void free_all(pg_solver *s)
+{
+    if (!s) return;
+    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_rtw); cudaFree(s->d_itw);
+    cudaFree(s->d_tw_col); cudaFree(s->d_mod); cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
+    cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); cudaFree(s->d_sigma_own); cudaFree(s->d_phi_own);
+    if (s->h_in) cudaFreeHost(s->h_in);
+    if (s->h_out) cudaFreeHost(s->h_out);
+    for (auto e : s->ev_in) if (e) cudaEventDestroy(e);
+    for (auto e : s->ev_solved) if (e) cudaEventDestroy(e);
+    for (auto e : s->ev_out) if (e) cudaEventDestroy(e);
+    if (s->ev_main) cudaEventDestroy(s->ev_main);
+    for (auto &q : s->prof_pool) for (int k = 0; k < 4; ++k) cudaEventDestroy(q.e[k]);
+    if (s->h2d) cudaStreamDestroy(s->h2d);
+    if (s->d2h) cudaStreamDestroy(s->d2h);
+    delete s;
+}
+
+pg_status create_impl(pg_solver *s)
+{
+    const int n_r = s->n_r, n_phi = s->n_phi;
+    int ndev = 0;
+    PG_CUDA(s, cudaGetDeviceCount(&ndev));
+    if (s->device < 0) PG_CUDA(s, cudaGetDevice(&s->device));
+    if (s->device >= ndev) { set_err(s, "device %d out of range (%d devices)", s->device, ndev); return PG_ERR_INVALID_ARG; }
+    PG_CUDA(s, cudaSetDevice(s->device));
+    cudaDeviceProp prop;
+    PG_CUDA(s, cudaGetDeviceProperties(&prop, s->device));
+    if (prop.major != 10) {
+        set_err(s, "device %d is sm_%d%d; this library is built for sm_100a (B200) only and has no fallback",
+                s->device, prop.major, prop.minor);
+        return PG_ERR_UNSUPPORTED;
+    }
+
+    s->du = std::log(s->r_out / s->r_in) / n_r;
+    s->dphi = 2.0 * M_PI / n_phi;
+    s->m_h = n_phi / 2 + 1;
+    const int C = pgk::cols_per_cta(n_r);
+    s->m_c = (s->m_h + C - 1) / C * C;
+    s->field = (size_t)n_r * n_phi;
+
+    // grid tables (A1, A2): geometric centres, exact sector areas in their sinh form
+    s->r.resize(n_r); s->dA.resize(n_r); s->phi.resize(n_phi);
+    std::vector<double> rs_in(n_r), rs_out(n_r), s2(n_phi);
+    {
+        const long double du = logl((long double)s->r_out / (long double)s->r_in) / n_r;
+        const long double dphi = 2.0L * kPiL / n_phi;
+        for (int i = 0; i < n_r; ++i) {
+            const long double ri = (long double)s->r_in * expl(((long double)i + 0.5L) * du);
+            s->r[i] = (double)ri;
+            s->dA[i] = (double)(ri * ri * sinhl(du) * dphi);
+            rs_in[i] = (double)(ri * sqrtl(ri));
+            rs_out[i] = (double)(1.0L / sqrtl(ri));
+        }
+        for (int j = 0; j < n_phi; ++j) {
+            s->phi[j] = (double)(((long double)j + 0.5L) * dphi);
+            const long double sn = sinl(kPiL * j / n_phi);
+            s2[j] = (double)(sn * sn);
+        }
+    }
+    // FFT tables
+    const int Lr = n_phi / 2;
+    std::vector<cplx> rtw(Lr), itw(Lr), mod(n_r);
+    for (int k = 0; k < Lr; ++k) {
+        const long double a = 2.0L * kPiL * k / n_phi;
+        rtw[k] = make_double2((double)(-0.5L * sinl(a)), (double)(-0.5L * cosl(a)));   // -(i/2) exp(-i a)
+        itw[k] = make_double2((double)(-sinl(a)), (double)cosl(a));                    //  i exp(+i a)
+    }
+    for (int n = 0; n < n_r; ++n) mod[n] = unit((long double)n / (2.0L * n_r));         // exp(-i pi n / n_r)
+
+    pg_status st;
+    if ((st = upload(s, &s->d_tw_row, fft_tables(Lr))) != PG_OK) return st;
+    if ((st = upload(s, &s->d_tw_col, fft_tables(n_r))) != PG_OK) return st;
+    if ((st = upload(s, &s->d_rtw, rtw)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_itw, itw)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_mod, mod)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_rs_in, rs_in)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_rs_out, rs_out)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_r, s->r)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_dA, s->dA)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_s2, s2)) != PG_OK) return st;
+
+    const size_t w_n = (size_t)s->max_batch * s->m_c * n_r;
+    PG_CUDA(s, cudaMalloc((void **)&s->d_W, w_n * sizeof(cplx)));
+    PG_CUDA(s, cudaMemset(s->d_W, 0, w_n * sizeof(cplx)));
+    PG_CUDA(s, cudaMalloc((void **)&s->d_khat, (size_t)s->m_c * 2 * n_r * sizeof(double)));
+
+    PG_CUDA(s, cudaStreamCreateWithFlags(&s->h2d, cudaStreamNonBlocking));
+    PG_CUDA(s, cudaStreamCreateWithFlags(&s->d2h, cudaStreamNonBlocking));
+    s->ev_in.assign(s->max_batch, nullptr);
+    s->ev_solved.assign(s->max_batch, nullptr);
+    s->ev_out.assign(s->max_batch, nullptr);
+    s->in_pending.assign(s->max_batch, 0);
+    for (int b = 0; b < s->max_batch; ++b) {
+        PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_in[b], cudaEventDisableTiming));
+        PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_solved[b], cudaEventDisableTiming));
+        PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_out[b], cudaEventDisableTiming));
+    }
+    PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_main, cudaEventDisableTiming));
+
+    if ((st = prepare_kernels_rows(s)) != PG_OK) return st;
+    if ((st = prepare_kernels_cols(s)) != PG_OK) return st;
+    return build_khat(s);
+}
+
+}  // namespace
+
+// =================================================================== C ABI
+extern "C" {
+
+pg_status pg_create_ex(pg_solver **out, int n_r, int n_phi, double r_in, double r_out, double eps, int max_batch,
+                       int device, void *cuda_stream)
+{
+    g_create_error[0] = 0;
+    if (!out) { set_err(nullptr, "out is NULL"); return PG_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!(r_in > 0.0) || !(r_out > r_in) || !(eps > 0.0) || !std::isfinite(r_out) || !std::isfinite(eps) ||
+        max_batch < 1) {
+        set_err(nullptr, "invalid argument: need 0 < r_in < r_out, eps > 0, max_batch >= 1");
+        return PG_ERR_INVALID_ARG;
+    }
+    if (!is_pow2(n_r) || !is_pow2(n_phi) || n_r < PG_MIN_N || n_phi < PG_MIN_N || n_r > PG_MAX_N ||
+        n_phi > PG_MAX_N) {
+        set_err(nullptr, "unsupported grid %dx%d: n_r and n_phi must be powers of two in [%d, %d]", n_r, n_phi,
+                PG_MIN_N, PG_MAX_N);
+        return PG_ERR_UNSUPPORTED;
+    }
+    pg_solver *s = new (std::nothrow) pg_solver;
+    if (!s) { set_err(nullptr, "out of host memory"); return PG_ERR_NOMEM; }
+    s->n_r = n_r; s->n_phi = n_phi; s->r_in = r_in; s->r_out = r_out; s->eps = eps;
+    s->max_batch = max_batch; s->device = device; s->stream = (cudaStream_t)cuda_stream;
+    pg_status st = create_impl(s);
+    if (st != PG_OK) {
+        snprintf(g_create_error, sizeof g_create_error, "%s", s->err);
+        free_all(s);
+        return st;
+    }
+    *out = s;
+    return PG_OK;
+}
+
+pg_status pg_create(pg_solver **out, int n_r, int n_phi, double r_in, double r_out, double eps)
+{
+    return pg_create_ex(out, n_r, n_phi, r_in, r_out, eps, 1, -1, nullptr);
+}
+
+pg_status pg_destroy(pg_solver *s)
+{
+    if (!s) return PG_OK;
+    cudaSetDevice(s->device);
+    cudaStreamSynchronize(s->stream);
+    if (s->h2d) cudaStreamSynchronize(s->h2d);
+    if (s->d2h) cudaStreamSynchronize(s->d2h);
+    free_all(s);
+    return PG_OK;
+}
+
+pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!sigma || batch < 1 || batch > s->max_batch) {
+        set_err(s, "pg_set_density: sigma is NULL or batch %d outside [1, %d]", batch, s->max_batch);
+        return PG_ERR_INVALID_ARG;
+    }
+    PG_CUDA(s, cudaSetDevice(s->device));
+    const size_t fbytes = s->field * sizeof(double);
+    if (where == PG_MEM_DEVICE) {
+        s->d_sigma = sigma;
+        s->sigma_from_host = false;
+    } else if (where == PG_MEM_HOST || where == PG_MEM_HOST_PINNED) {
+        pg_status st = ensure_staging(s, true, false);
+        if (st != PG_OK) return st;
+        if (where == PG_MEM_HOST && (st = ensure_pinned(s, true, false)) != PG_OK) return st;
+        // the owned device copy may still be read by solves already enqueued on the main stream
+        PG_CUDA(s, cudaEventRecord(s->ev_main, s->stream));
+        PG_CUDA(s, cudaStreamWaitEvent(s->h2d, s->ev_main, 0));
+        for (int b = 0; b < batch; ++b) {
+            const double *src = sigma + (size_t)b * s->field;
+            if (where == PG_MEM_HOST) {
+                double *stage = s->h_in + (size_t)b * s->field;
+                if (s->in_pending[b]) PG_CUDA(s, cudaEventSynchronize(s->ev_in[b]));   // slot still in flight
+                memcpy(stage, src, fbytes);
+                src = stage;
+            }
+            PG_CUDA(s, cudaMemcpyAsync(s->d_sigma_own + (size_t)b * s->field, src, fbytes, cudaMemcpyHostToDevice,
+                                       s->h2d));
+            PG_CUDA(s, cudaEventRecord(s->ev_in[b], s->h2d));
+            s->in_pending[b] = 1;
+        }
+        s->d_sigma = s->d_sigma_own;
+        s->sigma_from_host = true;
+    } else {
+        set_err(s, "pg_set_density: unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    s->cur_batch = batch;
+    return PG_OK;
+}
+
+static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memspace where, bool direct, int ring0,
+                                  int n_rings)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!phi) { set_err(s, "phi is NULL"); return PG_ERR_INVALID_ARG; }
+    if (s->cur_batch == 0 || !s->d_sigma) { set_err(s, "no density set: call pg_set_density first"); return PG_ERR_STATE; }
+    if (batch != s->cur_batch) {
+        set_err(s, "batch %d does not match the density's batch %d", batch, s->cur_batch);
+        return PG_ERR_INVALID_ARG;
+    }
+    if (where != PG_MEM_DEVICE && where != PG_MEM_HOST && where != PG_MEM_HOST_PINNED) {
+        set_err(s, "unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    PG_CUDA(s, cudaSetDevice(s->device));
+    const bool rings = n_rings >= 0;
+    if (rings && (ring0 < 0 || n_rings < 1 || ring0 + n_rings > s->n_r)) {
+        set_err(s, "ring range [%d, %d) outside [0, %d)", ring0, ring0 + n_rings, s->n_r);
+        return PG_ERR_INVALID_ARG;
+    }
+    const size_t out_field = rings ? (size_t)n_rings * s->n_phi : s->field;
+    const size_t obytes = out_field * sizeof(double);
+    const bool host_out = where != PG_MEM_DEVICE;
+    pg_status st;
+    if (host_out) {
+        if ((st = ensure_staging(s, false, true)) != PG_OK) return st;
+        if (where == PG_MEM_HOST && (st = ensure_pinned(s, false, true)) != PG_OK) return st;
+    }
+
+    if (!host_out && !s->sigma_from_host) {
+        // everything resident: one batched launch per kernel
+        if (direct) return launch_direct(s, s->d_sigma, phi, rings ? ring0 : 0, rings ? n_rings : s->n_r, batch);
+        return solve_fields(s, s->d_sigma, phi, s->d_W, batch);
+    }
+
+    // staged pipeline: field b is solved as soon as its H2D copy has landed, and copied back
+    // while field b+1 is being solved (copy streams h2d / d2h, compute on the caller's stream)
+    if (host_out) {
+        // previous D2H copies read d_phi_own
+        PG_CUDA(s, cudaEventRecord(s->ev_main, s->d2h));
+        PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_main, 0));
+    }
+    for (int b = 0; b < batch; ++b) {
+        if (s->sigma_from_host) PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_in[b], 0));
+        const double *sg = s->d_sigma + (size_t)b * s->field;
+        double *dst = host_out ? s->d_phi_own + (size_t)b * s->field : phi + (size_t)b * out_field;
+        if (direct) st = launch_direct(s, sg, dst, rings ? ring0 : 0, rings ? n_rings : s->n_r, 1);
+        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * s->m_c * s->n_r, 1);
+        if (st != PG_OK) return st;
+        if (host_out) {
+            PG_CUDA(s, cudaEventRecord(s->ev_solved[b], s->stream));
+            PG_CUDA(s, cudaStreamWaitEvent(s->d2h, s->ev_solved[b], 0));
+            double *hdst = (where == PG_MEM_HOST) ? s->h_out + (size_t)b * s->field : phi + (size_t)b * out_field;
+            PG_CUDA(s, cudaMemcpyAsync(hdst, dst, obytes, cudaMemcpyDeviceToHost, s->d2h));
+            PG_CUDA(s, cudaEventRecord(s->ev_out[b], s->d2h));
+        }
+    }
+    if (where == PG_MEM_HOST) {
+        for (int b = 0; b < batch; ++b) {
+            PG_CUDA(s, cudaEventSynchronize(s->ev_out[b]));
+            memcpy(phi + (size_t)b * out_field, s->h_out + (size_t)b * s->field, obytes);
+        }
+    }
+    return PG_OK;
+}
+
+pg_status pg_potential(pg_solver *s, double *phi, int batch, pg_memspace where)
+{
+    return potential_common(s, phi, batch, where, false, 0, -1);
+}
+
+pg_status pg_potential_direct(pg_solver *s, double *phi, int batch, pg_memspace where)
+{
+    return potential_common(s, phi, batch, where, true, 0, -1);
+}
+
+pg_status pg_potential_direct_rings(pg_solver *s, double *phi, int ring0, int n_rings, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (n_rings < 1) { set_err(s, "n_rings must be >= 1"); return PG_ERR_INVALID_ARG; }
+    const int saved = s->cur_batch;
+    if (saved == 0) { set_err(s, "no density set: call pg_set_density first"); return PG_ERR_STATE; }
+    s->cur_batch = 1;   // field 0 only
+    pg_status st = potential_common(s, phi, 1, where, true, ring0, n_rings);
+    s->cur_batch = saved;
+    return st;
+}
+
+pg_status pg_grid(const pg_solver *s, double *r, double *phi, double *cell_area)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (r) memcpy(r, s->r.data(), s->r.size() * sizeof(double));
+    if (phi) memcpy(phi, s->phi.data(), s->phi.size() * sizeof(double));
+    if (cell_area) memcpy(cell_area, s->dA.data(), s->dA.size() * sizeof(double));
+    return PG_OK;
+}
+
+pg_status pg_set_stream(pg_solver *s, void *cuda_stream)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    PG_CUDA(s, cudaSetDevice(s->device));
+    pg_status st = drain_profile(s);
+    if (st != PG_OK) return st;
+    PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    s->stream = (cudaStream_t)cuda_stream;
+    return PG_OK;
+}
+
+pg_status pg_synchronize(pg_solver *s)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    PG_CUDA(s, cudaSetDevice(s->device));
+    PG_CUDA(s, cudaStreamSynchronize(s->h2d));
+    PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    PG_CUDA(s, cudaStreamSynchronize(s->d2h));
+    return PG_OK;
+}
+
+pg_status pg_host_alloc(void **p, size_t bytes)
+{
+    if (!p || bytes == 0) return PG_ERR_INVALID_ARG;
+    *p = nullptr;
+    cudaError_t e = cudaHostAlloc(p, bytes, cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+        set_err(nullptr, "cudaHostAlloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? PG_ERR_NOMEM : PG_ERR_CUDA;
+    }
+    return PG_OK;
+}
+
+pg_status pg_host_free(void *p)
+{
+    if (!p) return PG_OK;
+    cudaError_t e = cudaFreeHost(p);
+    if (e != cudaSuccess) { set_err(nullptr, "cudaFreeHost failed: %s", cudaGetErrorString(e)); return PG_ERR_CUDA; }
+    return PG_OK;
+}
+
+pg_status pg_profile(pg_solver *s, int enable)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    pg_status st = drain_profile(s);
+    if (st != PG_OK) return st;
+    s->profile = enable != 0;
+    if (enable) for (int k = 0; k < PG_NUM_KERNELS; ++k) { s->prof_ms[k] = 0.0; s->prof_n[k] = 0; }
+    return PG_OK;
+}
+
+pg_status pg_kernel_times(pg_solver *s, double ms[PG_NUM_KERNELS], long launches[PG_NUM_KERNELS])
+{
+    if (!s || !ms || !launches) return PG_ERR_INVALID_ARG;
+    pg_status st = drain_profile(s);
+    if (st != PG_OK) return st;
+    for (int k = 0; k < PG_NUM_KERNELS; ++k) { ms[k] = s->prof_ms[k]; launches[k] = s->prof_n[k]; }
+    return PG_OK;
+}
+
+long pg_launch_count(const pg_solver *s) { return s ? s->launches : 0; }
+
+double pg_kernel_algorithmic_bytes(const pg_solver *s, int index, int batch)
+{
+    if (!s || batch < 1) return 0.0;
+    const double cells = (double)s->n_r * s->n_phi;
+    const double spec = 16.0 * s->n_r * s->m_h;          // one half-spectrum, complex128
+    const double khat = 8.0 * 2.0 * s->n_r * s->m_h;     // real spectrum of the padded kernel
+    switch (index) {
+        case 0: return batch * (8.0 * cells + spec);              // read Sigma, write W
+        case 1: return batch * (2.0 * spec) + khat;               // read W, write W, read Khat once
+        case 2: return batch * (spec + 8.0 * cells);              // read W, write Phi
+        default: return 0.0;
+    }
+}
+
+double pg_algorithmic_bytes(const pg_solver *s, int batch)
+{
+    return pg_kernel_algorithmic_bytes(s, 0, batch) + pg_kernel_algorithmic_bytes(s, 1, batch) +
+           pg_kernel_algorithmic_bytes(s, 2, batch);
+}
+
+const char *pg_status_string(pg_status st)
+{
+    switch (st) {
+        case PG_OK: return "PG_OK";
+        case PG_ERR_INVALID_ARG: return "PG_ERR_INVALID_ARG";
+        case PG_ERR_UNSUPPORTED: return "PG_ERR_UNSUPPORTED";
+        case PG_ERR_CUDA: return "PG_ERR_CUDA";
+        case PG_ERR_NOMEM: return "PG_ERR_NOMEM";
+        case PG_ERR_STATE: return "PG_ERR_STATE";
+    }
+    return "PG_ERR_UNKNOWN";
+}
+
+const char *pg_last_error(const pg_solver *s) { return s ? s->err : g_create_error; }
+
+const char *pg_version(void) { return "polargrav 0.1 (sm_100a)"; }
+
+}  // extern "C"
