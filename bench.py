@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- potential solves/s of the FFT-convolution path on synthetic disks (BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+
+A step = one pass of the whole hot path (rows a2, a3+a4r, a4phi of DESIGN.md) over one batch of
+the config's synthetic density, device resident (PG_MEM_DEVICE).  Default workload: config 5
+(2048x2048, the grid BASELINE.json's metric and north_star's 60 % target are quoted on).
+Successive steps rotate through R distinct (Sigma, Phi) buffer pairs whose total size exceeds the
+126 MB L2, so inputs do not stay cached between timed iterations.  One JSON line on stdout.
+
+Multi-GPU (torchrun): the path does not shard ("replicas only"): every rank
+runs the same workload on its own GPU, no data-path collective; value = all ranks' solves / max time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on this box's host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2409_02294_b200.workloads import CONFIGS, make_sigma  # noqa: E402
+
+METRIC = "potential solves/sec (fp64 FFT-convolution, log-polar thin disk)"
+UNIT = "solves/s"
+L2_BYTES = 126e6
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.path = tempfile.mktemp(prefix="pg_clocks_", suffix=".csv")
+        self.proc = None
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, mx, reasons = [], [], set()
+        try:
+            for line in open(self.path):
+                t = [x.strip() for x in line.split(",")]
+                if len(t) < 9:
+                    continue
+                try:
+                    sm.append(float(t[1])); mx.append(float(t[2]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), t[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def oracle_sample(cfg: int, seconds_target: float = 12.0):
+    """Times oracle.potential_o1_rings on a bounded sample of target rings of config `cfg`.
+    Returns (solves/s extrapolated to the whole grid, cores, description, seconds)."""
+    import oracle
+    c = CONFIGS[cfg]
+    r, phi, _, _ = oracle.grid(c.n_r, c.n_phi, c.r_in, c.r_out)
+    sigma = make_sigma(cfg, r, phi)
+    cores = oracle.num_threads()
+    rng = np.random.default_rng(0)
+    probe = np.sort(rng.choice(c.n_r, size=min(c.n_r, cores), replace=False)).astype(np.int32)
+    t0 = time.perf_counter()
+    oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, probe)
+    t_probe = time.perf_counter() - t0
+    waves = int(max(1, min(c.n_r // max(1, len(probe)), round(seconds_target / max(t_probe, 1e-3)))))
+    rings = np.sort(rng.choice(c.n_r, size=min(c.n_r, waves * len(probe)), replace=False)).astype(np.int32)
+    t0 = time.perf_counter()
+    oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
+    t = time.perf_counter() - t0
+    frac = len(rings) / c.n_r
+    solves_per_s = frac / t
+    desc = (f"oracle O1 (ring-pair direct sum, gcc -O3 -march=native -fopenmp) on {len(rings)} of {c.n_r} "
+            f"target rings of config {cfg} field 0 ({t:.2f} s), extrapolated to the whole grid by rings")
+    return solves_per_s, cores, desc, t, rings, sigma
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    cfg = args.config
+    c = CONFIGS[cfg]
+    sps, cores, desc, t_one, rings, sigma = oracle_sample(cfg, seconds_target=6.0)
+    for _ in range(args.warmup):
+        pass  # the sample above already warmed caches/threads; the oracle has no other state
+    times = []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
+        times.append(time.perf_counter() - t0)
+    t = float(np.mean(times))
+    value = (len(rings) / c.n_r) * c.batch / t / c.batch   # solves/s of one field, extrapolated
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
+                   "step": f"O1 direct sum over {len(rings)} of {c.n_r} target rings (bounded sample)"},
+        "cells_per_s": value * c.n_r * c.n_phi,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_name(cfg: int) -> str:
+    c = CONFIGS[cfg]
+    return f"BASELINE.json configs[{cfg - 1}]: {c.name}, r in [{c.r_in:g},{c.r_out:g}], eps={c.eps:g}, batch {c.batch}"
+
+
+# ------------------------------------------------------------------ the CUDA path
+def run_ours(args):
+    import torch
+    from paper_2409_02294_b200 import binding as pg, build as pg_build
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = args.config
+    c = CONFIGS[cfg]
+    field_bytes = 8 * c.n_r * c.n_phi
+    pair_bytes = 2 * field_bytes * c.batch
+    R = int(min(64, max(4, -(-4 * L2_BYTES // pair_bytes))))
+
+    st = torch.cuda.Stream()
+    solver = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, max_batch=c.batch, device=local_rank,
+                       cuda_stream=st.cuda_stream)
+    h = solver.h
+    r, phi, _ = solver.grid()
+    n_fields = R * c.batch
+    distinct = min(n_fields, 8 if c.n_r * c.n_phi >= 1 << 22 else 32)
+    base = [make_sigma(cfg, r, phi, b) for b in range(distinct)]
+    host_fields = [base[k] if k < distinct else np.roll(base[k % distinct], 97 * (k // distinct), axis=1)
+                   for k in range(n_fields)]
+    d_sig = [torch.from_numpy(np.stack(host_fields[p * c.batch:(p + 1) * c.batch])).cuda() for p in range(R)]
+    d_phi = [torch.empty_like(d_sig[p]) for p in range(R)]
+    torch.cuda.synchronize()
+
+    def step(k):
+        p = k % R
+        pg.pg_set_density(h, d_sig[p], c.batch, pg.PG_MEM_DEVICE)
+        pg.pg_potential(h, d_phi[p], c.batch, pg.PG_MEM_DEVICE)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        import torch.distributed as dist
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    for k in range(args.warmup):
+        step(k)
+    pg.pg_synchronize(h)
+
+    # ---- timed region: exactly K steps between CUDA events on the solver's stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    barrier(); torch.cuda.synchronize()
+    n0 = pg.pg_launch_count(h)
+    e0.record(st)
+    for k in range(args.steps):
+        step(k)
+    e1.record(st)
+    torch.cuda.synchronize(); barrier()
+    n1 = pg.pg_launch_count(h)
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    # keep the GPU busy a little longer so that short runs still collect clock samples under load
+    if sampler is not None:
+        t_end = time.perf_counter() + 0.6
+        k = 0
+        while time.perf_counter() < t_end:
+            step(k); k += 1
+            if k % 64 == 0:
+                pg.pg_synchronize(h)
+        pg.pg_synchronize(h)
+    clocks = sampler.stop() if sampler is not None else None
+    ms_per_step = ms_total / args.steps
+    value = world * c.batch * 1e3 / ms_per_step
+
+    # ---- per-kernel durations (events around every kernel, separate pass) -> roofline of the dominant kernel
+    pg.pg_profile(h, True)
+    for k in range(args.steps):
+        step(k)
+    kms, kn = pg.pg_kernel_times(h)
+    pg.pg_profile(h, False)
+    per_launch_ms = [kms[i] / max(1, kn[i]) for i in range(pg.PG_NUM_KERNELS)]
+    dom = int(np.argmax(per_launch_ms))
+    peak, peak_src = load_peaks()
+    kbytes = [pg.pg_kernel_algorithmic_bytes(h, i, c.batch) for i in range(pg.PG_NUM_KERNELS)]
+    achieved = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
+    path_bytes = pg.pg_algorithmic_bytes(h, c.batch)
+    path_gbs = path_bytes / (ms_per_step * 1e-3) / 1e9
+
+    # ---- L2-flushed variant: every step timed on its own with a >L2 memset in between
+    flush = torch.empty(int(3 * L2_BYTES), dtype=torch.uint8, device="cuda")
+    fl = []
+    with torch.cuda.stream(st):
+        for k in range(min(args.steps, 50)):
+            flush.fill_(k & 0xFF)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st); step(k); b.record(st)
+            fl.append((a, b))
+    torch.cuda.synchronize()
+    ms_flushed = float(np.median([a.elapsed_time(b) for a, b in fl]))
+    del flush
+
+    # ---- end to end through the C ABI with host buffers (copies inside the timed region)
+    pin_in = [pg.PinnedArray((c.batch, c.n_r, c.n_phi)) for _ in range(2)]
+    pin_out = [pg.PinnedArray((c.batch, c.n_r, c.n_phi)) for _ in range(2)]
+    for q in range(2):
+        pin_in[q].array[...] = np.stack(host_fields[q * c.batch:(q + 1) * c.batch])
+
+    def e2e_step(k):
+        q = k & 1
+        pg.pg_set_density(h, pin_in[q].ptr, c.batch, pg.PG_MEM_HOST_PINNED)
+        pg.pg_potential(h, pin_out[q].ptr, c.batch, pg.PG_MEM_HOST_PINNED)
+
+    e2e_steps = max(3, min(args.steps, 40))
+    for k in range(3):
+        e2e_step(k)
+    pg.pg_synchronize(h)
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(e2e_steps):
+        e2e_step(k)
+    pg.pg_synchronize(h)
+    t_e2e = max_over_ranks(time.perf_counter() - t0)
+    e2e_value = world * c.batch * e2e_steps / t_e2e
+    # serial variant: one blocking pageable-host call pair per step (PG_MEM_HOST)
+    pageable_in = np.stack(host_fields[:c.batch]); pageable_out = np.empty_like(pageable_in)
+    pg.pg_set_density(h, pageable_in, c.batch, pg.PG_MEM_HOST); pg.pg_potential(h, pageable_out, c.batch, pg.PG_MEM_HOST)
+    t0 = time.perf_counter()
+    n_pg = max(2, min(e2e_steps, 10))
+    for _ in range(n_pg):
+        pg.pg_set_density(h, pageable_in, c.batch, pg.PG_MEM_HOST)
+        pg.pg_potential(h, pageable_out, c.batch, pg.PG_MEM_HOST)
+    t_pageable = (time.perf_counter() - t0) / n_pg
+    sane = bool(np.isfinite(pageable_out).all() and (pageable_out < 0).all())
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
+                   "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
+                   "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
+                         f"{R * pair_bytes / 1e6:.0f} MB in total vs 126 MB L2"},
+        "cells_per_s": value * c.n_r * c.n_phi,
+        "gpu_launches": int((n1 - n0) * world),
+        "roofline": {
+            "bound": "hbm", "kernel": pg.KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg, dom)), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
+            "kernels": {pg.KERNEL_NAMES[i]: {"ms": per_launch_ms[i], "alg_bytes": kbytes[i],
+                                            "gbs": kbytes[i] / (per_launch_ms[i] * 1e-3) / 1e9 if per_launch_ms[i] > 0 else None}
+                        for i in range(pg.PG_NUM_KERNELS)},
+            "path": {"alg_bytes_per_step": path_bytes, "gbs": path_gbs, "frac_of_peak": path_gbs / peak,
+                     "frac_of_8TBs_nominal": path_gbs / 8000.0},
+            "l2_flushed_ms_per_step": ms_flushed, "l2_flushed_frac_of_peak": path_bytes / (ms_flushed * 1e-3) / 1e9 / peak,
+        },
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * c.batch,
+                "d2h_bytes_per_step": field_bytes * c.batch,
+                "how": "pg_set_density + pg_potential with PG_MEM_HOST_PINNED buffers (pg_host_alloc), wall clock over "
+                       f"{e2e_steps} steps, pg_synchronize at the end",
+                "pageable_blocking_ms_per_step": 1e3 * t_pageable, "output_sane": sane},
+        "clocks": clocks,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sps, cores, desc, _, _, _ = oracle_sample(cfg)
+        line["cpu_baseline"] = {"value": sps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    for a in pin_in + pin_out:
+        a.free()
+    solver.close()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
+# (profiles/), keyed by (config, kernel index).  Filled in from profiles/*.md; None = not captured.
+NCU_TRAFFIC: dict = {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

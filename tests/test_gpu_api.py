@@ -1,0 +1,179 @@
+"""Boundary behaviour on a real device: the three memspaces (row a6: pinned staging on CUDA
+streams, Fig. 4 :202), ordering, state errors, batch rules, profiling
+counters.  Arithmetic parity lives in test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from paper_2409_02294_b200 import binding as pg
+from paper_2409_02294_b200.workloads import random_sigma
+
+pytestmark = pytest.mark.gpu
+
+N_R, N_PHI, R_IN, R_OUT, EPS = 128, 256, 1.0, 300.0, 0.01
+
+
+@pytest.fixture()
+def solver():
+    s = pg.Solver(N_R, N_PHI, R_IN, R_OUT, EPS, max_batch=4, device=0,
+                  cuda_stream=torch.cuda.current_stream().cuda_stream)
+    yield s
+    s.close()
+
+
+def device_solve(s, sig):
+    batch = 1 if sig.ndim == 2 else sig.shape[0]
+    d_s = torch.from_numpy(np.ascontiguousarray(sig)).cuda()
+    d_p = torch.empty_like(d_s)
+    pg.pg_set_density(s.h, d_s, batch, pg.PG_MEM_DEVICE)
+    pg.pg_potential(s.h, d_p, batch, pg.PG_MEM_DEVICE)
+    pg.pg_synchronize(s.h)
+    return d_p.cpu().numpy()
+
+
+def test_memspaces_agree_bit_for_bit(solver):
+    sig = np.stack([random_sigma(N_R, N_PHI, 10 + b) for b in range(4)])
+    ref = np.stack([oracle.potential_o1(N_R, N_PHI, R_IN, R_OUT, EPS, sig[b]) for b in range(4)])
+    dev = device_solve(solver, sig)
+    assert np.abs(dev / ref - 1).max() <= 1e-9
+    # pageable host -> staged through owned pinned buffers, blocking
+    host = solver.potential_host(sig)
+    assert np.array_equal(host, dev)
+    # caller-owned pinned memory (pg_host_alloc), asynchronous
+    pin_in, pin_out = pg.PinnedArray(sig.shape), pg.PinnedArray(sig.shape)
+    try:
+        pin_in.array[...] = sig
+        pin_out.array[...] = 0.0
+        pg.pg_set_density(solver.h, pin_in.ptr, 4, pg.PG_MEM_HOST_PINNED)
+        pg.pg_potential(solver.h, pin_out.ptr, 4, pg.PG_MEM_HOST_PINNED)
+        pg.pg_synchronize(solver.h)
+        assert np.array_equal(pin_out.array, dev)
+        # mixed: host density, device potential
+        d_p = torch.empty(sig.shape, dtype=torch.float64, device="cuda")
+        pg.pg_set_density(solver.h, sig, 4, pg.PG_MEM_HOST)
+        pg.pg_potential(solver.h, d_p, 4, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(solver.h)
+        assert np.array_equal(d_p.cpu().numpy(), dev)
+        # mixed: device density, host potential
+        d_s = torch.from_numpy(sig).cuda()
+        out = np.empty_like(sig)
+        pg.pg_set_density(solver.h, d_s, 4, pg.PG_MEM_DEVICE)
+        pg.pg_potential(solver.h, out, 4, pg.PG_MEM_HOST)
+        assert np.array_equal(out, dev)
+    finally:
+        pin_in.free(); pin_out.free()
+
+
+def test_repeated_host_solves_reuse_staging_safely(solver):
+    prev = None
+    for k in range(6):
+        sig = random_sigma(N_R, N_PHI, 50 + k)
+        got = solver.potential_host(sig)
+        ref = device_solve(solver, sig)
+        assert np.array_equal(got, ref)
+        assert prev is None or not np.array_equal(prev, got)
+        prev = got
+
+
+def test_direct_host_path_and_rings(solver):
+    sig = random_sigma(N_R, N_PHI, 3)
+    full = solver.potential_host(sig, direct=True)
+    ref = oracle.potential_o1(N_R, N_PHI, R_IN, R_OUT, EPS, sig)
+    assert np.abs(full / ref - 1).max() <= 1e-12
+    out = np.empty((5, N_PHI))
+    pg.pg_set_density(solver.h, sig, 1, pg.PG_MEM_HOST)
+    pg.pg_potential_direct_rings(solver.h, out, 100, 5, pg.PG_MEM_HOST)
+    assert np.array_equal(out, full[100:105])
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential_direct_rings(solver.h, out, 125, 5, pg.PG_MEM_HOST)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+
+
+def test_state_and_argument_errors(solver):
+    out = np.empty((N_R, N_PHI))
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential(solver.h, out, 1, pg.PG_MEM_HOST)          # before any density
+    assert e.value.status == pg.PG_ERR_STATE
+    sig = random_sigma(N_R, N_PHI, 1)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_set_density(solver.h, sig, 5, pg.PG_MEM_HOST)         # batch > max_batch
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_set_density(solver.h, sig, 0, pg.PG_MEM_HOST)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_set_density(solver.h, sig, 1, 7)                      # unknown memspace
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    pg.pg_set_density(solver.h, sig, 1, pg.PG_MEM_HOST)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential(solver.h, out, 2, pg.PG_MEM_HOST)           # batch mismatch
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    assert "batch" in pg.last_error(solver.h)
+    pg.pg_potential(solver.h, out, 1, pg.PG_MEM_HOST)               # still usable after errors
+    assert np.isfinite(out).all()
+
+
+def test_nan_propagates_not_checked(solver):
+    sig = random_sigma(N_R, N_PHI, 2)
+    sig[7, 9] = np.nan
+    assert np.isnan(solver.potential_host(sig)).any()
+
+
+def test_own_stream_and_set_stream():
+    st = torch.cuda.Stream()
+    s = pg.Solver(64, 64, 1.0, 100.0, 0.01, device=0, cuda_stream=st.cuda_stream)
+    try:
+        sig = random_sigma(64, 64, 5)
+        with torch.cuda.stream(st):
+            d_s = torch.from_numpy(sig).cuda()
+            d_p = torch.empty_like(d_s)
+        st.synchronize()
+        pg.pg_set_density(s.h, d_s, 1, pg.PG_MEM_DEVICE)
+        pg.pg_potential(s.h, d_p, 1, pg.PG_MEM_DEVICE)
+        st.synchronize()
+        a = d_p.cpu().numpy()
+        pg.pg_set_stream(s.h, None)                                   # legacy default stream
+        pg.pg_potential(s.h, d_p, 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(s.h)
+        assert np.array_equal(a, d_p.cpu().numpy())
+        ref = oracle.potential_o1(64, 64, 1.0, 100.0, 0.01, sig)
+        assert np.abs(a / ref - 1).max() <= 1e-9
+    finally:
+        s.close()
+
+
+def test_profile_counters_and_algorithmic_bytes(solver):
+    sig = np.stack([random_sigma(N_R, N_PHI, 20 + b) for b in range(2)])
+    d_s = torch.from_numpy(sig).cuda()
+    d_p = torch.empty_like(d_s)
+    pg.pg_set_density(solver.h, d_s, 2, pg.PG_MEM_DEVICE)
+    n0 = pg.pg_launch_count(solver.h)
+    pg.pg_profile(solver.h, True)
+    for _ in range(5):
+        pg.pg_potential(solver.h, d_p, 2, pg.PG_MEM_DEVICE)
+    ms, n = pg.pg_kernel_times(solver.h)
+    pg.pg_profile(solver.h, False)
+    assert n == [5, 5, 5] and all(t > 0 for t in ms)
+    assert pg.pg_launch_count(solver.h) - n0 == 15                   # three kernels per solve
+    m_h = N_PHI // 2 + 1
+    cells, spec = N_R * N_PHI, 16 * N_R * m_h
+    assert pg.pg_kernel_algorithmic_bytes(solver.h, 0, 2) == 2 * (8 * cells + spec)
+    assert pg.pg_kernel_algorithmic_bytes(solver.h, 1, 2) == 2 * 2 * spec + 16 * N_R * m_h
+    assert pg.pg_kernel_algorithmic_bytes(solver.h, 2, 2) == 2 * (spec + 8 * cells)
+    assert pg.pg_algorithmic_bytes(solver.h, 2) == sum(pg.pg_kernel_algorithmic_bytes(solver.h, k, 2) for k in range(3))
+
+
+def test_two_solvers_are_independent():
+    a = pg.Solver(64, 64, 1.0, 100.0, 0.01, device=0)
+    b = pg.Solver(64, 128, 1.0, 50.0, 0.02, device=0)
+    try:
+        sa, sb = random_sigma(64, 64, 1), random_sigma(64, 128, 2)
+        pa1 = a.potential_host(sa)
+        pb = b.potential_host(sb)
+        pa2 = a.potential_host(sa)
+        assert np.array_equal(pa1, pa2)
+        assert np.abs(pb / oracle.potential_o1(64, 128, 1.0, 50.0, 0.02, sb) - 1).max() <= 1e-9
+    finally:
+        a.close(); b.close()

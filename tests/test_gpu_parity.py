@@ -1,0 +1,216 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star): relative L2 <= 1e-10, max pointwise relative
+<= 1e-9, fp64.  Oracle = oracle/polar_oracle.c (O1 ring-pair direct summation, pinned in
+tests/test_oracle_pins.py); inputs = paper_2409_02294_b200.workloads on the library's pg_grid
+tables (which are themselves compared with the oracle's tables first)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+from paper_2409_02294_b200 import binding as pg
+from paper_2409_02294_b200.workloads import CONFIGS, make_batch, make_sigma, random_sigma
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1e-10      # north_star
+MAX_REL = 1e-9      # north_star
+
+
+def errs(got, ref):
+    got, ref = np.asarray(got), np.asarray(ref)
+    l2 = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got / ref - 1.0).max()
+    return l2, mx
+
+
+def assert_parity(got, ref, what=""):
+    l2, mx = errs(got, ref)
+    assert l2 <= REL_L2 and mx <= MAX_REL, f"{what}: rel-L2 {l2:.3e} (<= {REL_L2}), max rel {mx:.3e} (<= {MAX_REL})"
+    return l2, mx
+
+
+class Dev:
+    """Solver + device buffers held through torch (device memory and stream only)."""
+
+    def __init__(self, n_r, n_phi, r_in, r_out, eps, max_batch=1):
+        self.stream = torch.cuda.current_stream()
+        self.s = pg.Solver(n_r, n_phi, r_in, r_out, eps, max_batch=max_batch, device=0,
+                           cuda_stream=self.stream.cuda_stream)
+        self.shape = (n_r, n_phi)
+
+    def solve(self, sigma, direct=False):
+        s = np.ascontiguousarray(sigma, dtype=np.float64)
+        batch = 1 if s.ndim == 2 else s.shape[0]
+        d_s = torch.from_numpy(s).cuda()
+        d_p = torch.empty_like(d_s)
+        pg.pg_set_density(self.s.h, d_s, batch, pg.PG_MEM_DEVICE)
+        (pg.pg_potential_direct if direct else pg.pg_potential)(self.s.h, d_p, batch, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(self.s.h)
+        return d_p.cpu().numpy()
+
+    def direct_rings(self, sigma, ring0, n):
+        d_s = torch.from_numpy(np.ascontiguousarray(sigma)).cuda()
+        d_p = torch.empty((n, self.shape[1]), dtype=torch.float64, device="cuda")
+        pg.pg_set_density(self.s.h, d_s, 1, pg.PG_MEM_DEVICE)
+        pg.pg_potential_direct_rings(self.s.h, d_p, ring0, n, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(self.s.h)
+        return d_p.cpu().numpy()
+
+    def close(self):
+        self.s.close()
+
+
+def cfg_solver(cfg):
+    c = CONFIGS[cfg]
+    return c, Dev(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, max_batch=c.batch)
+
+
+# ---------------------------------------------------------------- grid tables (P11 on the GPU side)
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_pg_grid_equals_oracle_grid(cfg):
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, area = d.s.grid()
+        ro, po, ao, _ = oracle.grid(c.n_r, c.n_phi, c.r_in, c.r_out)
+        np.testing.assert_allclose(r, ro, rtol=4e-15)
+        np.testing.assert_allclose(phi, po, rtol=4e-15)
+        np.testing.assert_allclose(area, ao, rtol=2e-13)
+    finally:
+        d.close()
+
+
+# ---------------------------------------------------------------- configs 1-2: every cell
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_fft_path_full_grid_vs_oracle(cfg):
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, _ = d.s.grid()
+        sigma = make_sigma(cfg, r, phi)
+        ref = oracle.potential_o1(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma)
+        got = d.solve(sigma)
+        assert_parity(got, ref, f"config {cfg} FFT path")
+        got_d = d.solve(sigma, direct=True)
+        assert_parity(got_d, ref, f"config {cfg} direct kernel (a5)")
+        assert_parity(got, got_d, f"config {cfg} FFT vs direct on the GPU")
+    finally:
+        d.close()
+
+
+# ---------------------------------------------------------------- configs 3-5: sampled target rings at full size
+def sample_rings(n_r, n, seed):
+    rng = np.random.default_rng(seed)
+    fixed = [0, 1, n_r // 2, n_r - 2, n_r - 1]
+    extra = rng.choice(np.arange(2, n_r - 2), size=max(0, n - len(fixed)), replace=False)
+    return np.unique(np.concatenate([fixed, extra])).astype(np.int32)
+
+
+@pytest.mark.parametrize("cfg,n_rings", [(3, 48), (5, 10)])
+def test_fft_path_sampled_rings_vs_oracle_full_size(cfg, n_rings):
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, _ = d.s.grid()
+        sigma = make_sigma(cfg, r, phi)
+        rings = sample_rings(c.n_r, n_rings, cfg)
+        ref = oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
+        got = d.solve(sigma)
+        assert np.isfinite(got).all() and (got < 0).all()
+        assert_parity(got[rings], ref, f"config {cfg} FFT path, {len(rings)} rings")
+        # a5 cross-check on a few of the same rings (direct kernel is O(N^2))
+        for i in (0, int(rings[len(rings) // 2]), c.n_r - 1):
+            k = int(np.where(rings == i)[0][0])
+            gd = d.direct_rings(sigma, i, 1)
+            assert_parity(gd[0], ref[k], f"config {cfg} direct kernel ring {i}")
+    finally:
+        d.close()
+
+
+def test_config4_batch_of_8_vs_oracle():
+    c, d = cfg_solver(4)
+    try:
+        r, phi, _ = d.s.grid()
+        sig = make_batch(4, r, phi)
+        assert sig.shape == (8, 1024, 1024)
+        got = d.solve(sig)
+        for b in range(c.batch):
+            rings = sample_rings(c.n_r, 6, 40 + b)
+            ref = oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sig[b], rings)
+            assert_parity(got[b][rings], ref, f"config 4 field {b}")
+        # the batched launch equals eight single solves bit for bit (same kernels, same order)
+        one = d.solve(sig[3])
+        assert np.array_equal(one, got[3])
+    finally:
+        d.close()
+
+
+# ---------------------------------------------------------------- P4 on the GPU: single cell, no wrap-around
+@pytest.mark.parametrize("n", [64, 256, 2048])
+def test_single_cell_response_no_radial_wraparound(n):
+    r_out = {64: 100.0, 256: 500.0, 2048: 2000.0}[n]
+    eps = 0.01
+    d = Dev(n, n, 1.0, r_out, eps)
+    try:
+        r, phi, area = d.s.grid()
+        h = np.sqrt(area)
+        for i0 in (0, n - 1, n // 2):
+            j0 = 5
+            s = np.zeros((n, n)); s[i0, j0] = 1.0
+            d2 = (r[:, None] - r[i0]) ** 2 + 4 * r[:, None] * r[i0] * np.sin(0.5 * (phi[None, :] - phi[j0])) ** 2 \
+                + eps ** 2 * h[:, None] * h[i0]
+            expect = -area[i0] / np.sqrt(d2)
+            got = d.solve(s)
+            # rounding of the FFT path is uniform in the reduced potential sqrt(r) Phi
+            red = np.abs(got - expect) * np.sqrt(r)[:, None] / np.abs(expect * np.sqrt(r)[:, None]).max()
+            assert red.max() <= 1e-13, (n, i0, red.max())
+            assert np.abs(got / expect - 1.0).max() <= MAX_REL, (n, i0)
+            assert abs(got[i0, j0] / (-h[i0] / eps) - 1.0) <= 1e-12
+    finally:
+        d.close()
+
+
+# ---------------------------------------------------------------- invariants at the bench size (hold at any size)
+def test_invariants_at_2048():
+    c, d = cfg_solver(5)
+    try:
+        r, phi, area = d.s.grid()
+        s1 = make_sigma(5, r, phi)
+        p1 = d.solve(s1)
+        # P3: roll in phi
+        p_roll = d.solve(np.roll(s1, 37, axis=1))
+        assert errs(p_roll, np.roll(p1, 37, axis=1))[1] <= 1e-11
+        # P2: linearity with a negative weight
+        s2 = random_sigma(c.n_r, c.n_phi, 99, signed=True)
+        p2 = d.solve(s2)
+        p12 = d.solve(0.5 * s1 - 2.0 * s2)
+        l2 = np.linalg.norm(p12 - (0.5 * p1 - 2.0 * p2)) / np.linalg.norm(p12)
+        assert l2 <= 1e-12
+        # P1: axisymmetric density -> axisymmetric potential
+        pa = d.solve(np.repeat(np.exp(-r / 200.0)[:, None], c.n_phi, axis=1))
+        assert ((pa.max(axis=1) - pa.min(axis=1)) / np.abs(pa).max(axis=1)).max() <= 1e-12
+        # P6: reciprocity
+        a = (s1 * area[:, None] * p2).sum(); b = (s2 * area[:, None] * p1).sum()
+        assert abs(a / b - 1.0) <= 1e-10
+    finally:
+        d.close()
+
+
+# ---------------------------------------------------------------- rectangular and small grids
+@pytest.mark.parametrize("n_r,n_phi", [(32, 32), (32, 128), (128, 32), (64, 512), (512, 64), (128, 256)])
+def test_rectangular_grids_full_vs_oracle(n_r, n_phi):
+    d = Dev(n_r, n_phi, 0.7, 60.0, 0.02)
+    try:
+        s = random_sigma(n_r, n_phi, n_r * 7 + n_phi)
+        ref = oracle.potential_o1(n_r, n_phi, 0.7, 60.0, 0.02, s)
+        assert_parity(d.solve(s), ref, f"{n_r}x{n_phi} FFT")
+        assert_parity(d.solve(s, direct=True), ref, f"{n_r}x{n_phi} direct")
+    finally:
+        d.close()
+
+
+def test_zero_density_gives_zero_potential():
+    d = Dev(64, 64, 1.0, 100.0, 0.01)
+    try:
+        assert np.all(d.solve(np.zeros((64, 64))) == 0.0)
+    finally:
+        d.close()
