@@ -9,12 +9,22 @@
 // Element distribution: thread u holds indices u + T*jj (jj = 0..15) on input AND on output,
 // for both directions, so global loads/stores are coalesced and the forward spectrum can be
 // consumed by the inverse transform without any reordering (PAPER.md:19 names "FFT
-// operations" as the GPU-resident work; the decomposition is ours, DESIGN.md section 5).
+// operations" as the GPU-resident work; the decomposition is ours, DESIGN.md section 7).
 //
-// Twiddle tables are read-only global arrays built on the host in long double:
-//   tw0[k1*(L/R1) + b]  = exp(-2 pi i b k1 / L),        k1 in [0,R1), b in [0,L/R1)   (if R1 > 1)
-//   tw1[k*T3 + t]       = exp(-2 pi i t k / (L/R1)),    k in [0,16),  t in [0,T3=L/(16 R1)) (if n16 == 2)
-// laid out as [tw0 | tw1].
+// Twiddles.  The first version of this file read every inter-pass twiddle from a global table
+// (29 16-byte loads per thread and transform at L = 2048).  ncu showed the L1TEX data pipe as the
+// busiest unit of all three kernels with ~40 % of its wavefronts spent on those table reads, and
+// their L1/L2 latency exposed once per pass (profiles/r1_01_baseline.md).  Now a thread loads only
+// its BASE roots once (Twid<L>: w_L^(u + T m) for the leading pass, w_T2^t for the radix-16 link)
+// from one unit-root table  root[b * rs] = exp(-2 pi i b / L)  built on the host in long double,
+// and forms the powers it needs by two interleaved multiplication chains (step p^2), which costs
+// ~16 % more FP64 instructions but no table traffic.  Chains are at most 7 products deep: the
+// twiddle error stays below ~10 ulp, far inside the 1e-10 parity bar.
+//
+// The transform is split into a HEAD (everything up to the stores of the last exchange) and a
+// LAST pass (16 consecutive slots -> radix-16), so that a kernel may hand the last pass to a
+// different thread than the one that ran the head (rows kernels: row-fastest mapping for a
+// coalesced transposed store without an extra shared-memory transposition).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -34,18 +44,23 @@ __device__ __forceinline__ cplx cmulc(cplx a, cplx w)
 {
     return make_double2(fma(a.y, w.y, a.x * w.x), fma(a.y, w.x, -(a.x * w.y)));
 }
-
-// Table load.  Deliberately a plain (coherent) ld.global, not ld.global.nc / __ldg: ptxas hoists
-// non-coherent loads across bar.sync all the way to the kernel entry, which put every twiddle of
-// every pass in flight at once and spilled them (measured: 300-680 bytes of spills at 128
-// registers).  A coherent load cannot cross a barrier, so each pass loads its own twiddles while
-// the previous butterfly computes.  The tables stay L1/L2 resident either way.
-__device__ __forceinline__ cplx ld_table(const cplx *p)
+// w * w
+__device__ __forceinline__ cplx csq(cplx w)
 {
-    cplx r;
-    asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
+    const double t = w.x * w.y;
+    return make_double2(fma(w.x, w.x, -(w.y * w.y)), t + t);
 }
+// acc + a * w
+__device__ __forceinline__ cplx cfma(cplx a, cplx w, cplx acc)
+{
+    return make_double2(fma(-a.y, w.y, fma(a.x, w.x, acc.x)), fma(a.y, w.x, fma(a.x, w.y, acc.y)));
+}
+// acc + conj(a) * w
+__device__ __forceinline__ cplx cfmac(cplx a, cplx w, cplx acc)
+{
+    return make_double2(fma(a.y, w.y, fma(a.x, w.x, acc.x)), fma(-a.y, w.x, fma(a.x, w.y, acc.y)));
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
 
 __host__ __device__ constexpr int pad_idx(int a) { return a + (a >> 4); }
 
@@ -146,36 +161,49 @@ struct Plan {
     static constexpr int T = L / 16;                         // threads per transform
     static constexpr int N16 = (L >= 256) ? 2 : 1;           // number of radix-16 passes
     static constexpr int R1 = L / (N16 == 2 ? 256 : 16);     // leading small radix (1 = absent)
+    static constexpr int M = 16 / R1;                        // butterflies per thread in the leading pass
     static constexpr int T2 = L / R1;                        // sub-length after the leading pass
     static constexpr int T3 = T2 / 16;                       // sub-length after the first radix-16 pass
-    static constexpr int TW0 = (R1 > 1) ? L : 0;             // entries in tw0
-    static constexpr int TW1 = (N16 == 2) ? T2 : 0;          // entries in tw1
-    static constexpr int TW = TW0 + TW1;
+    static constexpr int NLEAD = (R1 > 1) ? M : 1;           // base roots held for the leading pass
     static constexpr int LINE = pad_idx(L) + 8;              // smem slots per transform (>= pad_idx(L)+1)
+    static constexpr bool HAS_EXCHANGE = (L > 16);           // false: the whole transform is one radix-16
 };
 
-// CTA-wide barrier used between exchange phases.  All threads of the CTA must call the
-// transforms together.
-__device__ __forceinline__ void cta_sync() { __syncthreads(); }
+// ------------------------------------------------------------------ barriers
+// Sync<T, CTA>: barrier among the T threads of one transform.  When a transform is made of whole
+// warps (T >= 32) and the CTA holds several transforms, each gets its own named barrier
+// (bar.sync id, T), so that the transforms of a CTA drift apart instead of marching in lockstep;
+// otherwise the CTA-wide barrier is used (every thread of the CTA then runs the same sequence).
+template <int T, int CTA_THREADS>
+struct Sync {
+    static constexpr bool NAMED = (T >= 32) && (T < CTA_THREADS) && (CTA_THREADS / T <= 15);
+    int id;
+    __device__ __forceinline__ explicit Sync(int group) : id(group + 1) {}
+    __device__ __forceinline__ void operator()() const
+    {
+        if constexpr (NAMED) asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(T) : "memory");
+        else __syncthreads();
+    }
+};
 
 // ------------------------------------------------------------------ shared-memory addressing
 // Every exchange address is written as (per-thread base) + (compile-time constant), so that the
 // forward and the inverse transform of one kernel share three base registers instead of keeping
-// dozens of computed addresses alive (which spilled at 128 registers per thread).
+// dozens of computed addresses alive.
 //   pad_idx(a + c) = pad_idx(a) + c + c/16            when c is a multiple of 16
 //   pad_idx(16 a + j) = 17 a + j                      for 0 <= j < 16
 template <int L>
 struct Lines {
     typedef Plan<L> P;
     cplx *lin;   // sm + pad_idx(u)            consecutive-lane side of the radix-16 exchanges
-    cplx *blk;   // sm + 17 u                  16 consecutive slots of the last radix-16 pass
     cplx *mid;   // sm + pad_idx(q T2 + t)     strided side of the leading-pass exchange
     __device__ __forceinline__ Lines(cplx *sm, int u)
     {
         lin = sm + (P::N16 == 2 ? pad_idx(u) : u);
-        blk = sm + 17 * u;
-        mid = (P::N16 == 2) ? sm + (u / P::T3) * pad_idx(P::T2) + (u % P::T3) : blk;
+        mid = (P::N16 == 2) ? sm + (u / P::T3) * pad_idx(P::T2) + (u % P::T3) : sm + 17 * u;
     }
+    // 16 consecutive slots of the last radix-16 pass of thread u
+    static __device__ __forceinline__ cplx *blk(cplx *sm, int u) { return sm + 17 * u; }
     // leading pass, element (k, b = u + T m):  pad_idx(k T2 + b)
     static __host__ __device__ constexpr int lead(int k, int m)
     {
@@ -187,93 +215,171 @@ struct Lines {
     static __host__ __device__ constexpr int link(int k) { return pad_idx(P::T * k); }
 };
 
+// ------------------------------------------------------------------ twiddle bases and powers
+// root[b * rs] = exp(-2 pi i b / L) for 0 <= b < L  (rs = table length / L)
+template <int L>
+struct Twid {
+    typedef Plan<L> P;
+    cplx lead[P::NLEAD];   // w_L^(u + T m), m < M            (R1 > 1)
+    cplx link;             // w_T2^t = w_L^(R1 t), t = u % T3  (N16 == 2)
+    __device__ __forceinline__ void load(const cplx *__restrict__ root, const int rs, const int u)
+    {
+        if constexpr (P::R1 > 1) {
+#pragma unroll
+            for (int m = 0; m < P::M; ++m) lead[m] = __ldg(&root[(u + P::T * m) * rs]);
+        }
+        if constexpr (P::N16 == 2) link = __ldg(&root[(u % P::T3) * P::R1 * rs]);
+    }
+};
+
+// x[k] *= p^k (CONJ: conj(p)^k) for k = 1..K-1.  Two interleaved chains a = p^(odd), b = p^(even),
+// both advanced by p^2: depth K/2, three live roots.
+template <int K, bool CONJ>
+__device__ __forceinline__ void apply_powers(cplx *x, const cplx p)
+{
+    if constexpr (K >= 2) {
+        x[1] = CONJ ? cmulc(x[1], p) : cmul(x[1], p);
+        if constexpr (K > 2) {
+            const cplx p2 = csq(p);
+            cplx a = p, b = p2;
+            x[2] = CONJ ? cmulc(x[2], b) : cmul(x[2], b);
+#pragma unroll
+            for (int k = 3; k < K; k += 2) {
+                a = cmul(a, p2);
+                x[k] = CONJ ? cmulc(x[k], a) : cmul(x[k], a);
+                if (k + 1 < K) {
+                    b = cmul(b, p2);
+                    x[k + 1] = CONJ ? cmulc(x[k + 1], b) : cmul(x[k + 1], b);
+                }
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------ forward transform
 // v[jj] = x[u + T*jj]  ->  v[k] = X[u + T*k],  X[k] = sum_n x[n] exp(-2 pi i n k / L)
-template <int L>
-__device__ __forceinline__ void fft_fwd(cplx (&v)[16], cplx *__restrict__ sm, const cplx *__restrict__ tw,
-                                        const int u)
+//
+// fwd_head: all passes but the last, ending with the STORES of the last exchange (no barrier).
+// fwd_last: after a barrier that covers those stores, thread u' of the transform whose line is
+//           `sm` reads its 16 slots and runs the last radix-16: v[k] = X[u' + T*k].
+// For L == 16 the head is empty and fwd_last transforms the registers it is given.
+template <int L, class SyncT>
+__device__ __forceinline__ void fwd_head(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
+                                         const SyncT &sync)
 {
     typedef Plan<L> P;
     typedef Lines<L> A;
-    constexpr int T = P::T, R1 = P::R1, T2 = P::T2, T3 = P::T3;
+    constexpr int T = P::T, R1 = P::R1, M = P::M;
+    (void)T;
     const A a(sm, u);
     if constexpr (R1 > 1) {
-        constexpr int M = 16 / R1;   // butterflies per thread in the leading pass
 #pragma unroll
         for (int m = 0; m < M; ++m) {
             cplx x[R1];
 #pragma unroll
             for (int j = 0; j < R1; ++j) x[j] = v[m + M * j];
             dft<R1, false>(x);
-            const cplx *twb = tw + u + T * m;
-#pragma unroll
-            for (int k = 1; k < R1; ++k) x[k] = cmul(x[k], ld_table(&twb[k * T2]));
+            apply_powers<R1, false>(x, tw.lead[m]);
 #pragma unroll
             for (int k = 0; k < R1; ++k) a.lin[A::lead(k, m)] = x[k];
         }
-        cta_sync();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = a.mid[A::midj(j)];
-        cta_sync();
     }
-    dft<16, false>(v);
     if constexpr (P::N16 == 2) {
-        const cplx *tw1 = tw + P::TW0 + (u % T3);
+        if constexpr (R1 > 1) {
+            sync();
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmul(v[k], ld_table(&tw1[k * T3]));
+            for (int j = 0; j < 16; ++j) v[j] = a.mid[A::midj(j)];
+            sync();
+        }
+        dft<16, false>(v);
+        apply_powers<16, false>(v, tw.link);
 #pragma unroll
         for (int k = 0; k < 16; ++k) a.lin[A::link(k)] = v[k];
-        cta_sync();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = a.blk[j];
-        cta_sync();
-        dft<16, false>(v);
     }
+}
+
+template <int L>
+__device__ __forceinline__ void fwd_last(cplx (&v)[16], const cplx *__restrict__ sm, const int u)
+{
+    if constexpr (Plan<L>::HAS_EXCHANGE) {
+        const cplx *b = sm + 17 * u;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) v[j] = b[j];
+    }
+    dft<16, false>(v);
 }
 
 // ------------------------------------------------------------------ inverse transform (unnormalised)
 // v[k] = X[u + T*k]  ->  v[jj] = sum_k X[k] exp(+2 pi i n k / L),  n = u + T*jj
-// Exact transpose of fft_fwd's flow graph, with conjugated twiddles.
+// Exact transpose of the forward flow graph, with conjugated twiddles.
+//
+// inv_first: radix-16 on X[u' + T*k] and the stores of the first exchange (no barrier).
+// inv_tail : after a barrier, thread u finishes the transform.
 template <int L>
-__device__ __forceinline__ void fft_inv(cplx (&v)[16], cplx *__restrict__ sm, const cplx *__restrict__ tw,
-                                        const int u)
+__device__ __forceinline__ void inv_first(cplx (&v)[16], cplx *__restrict__ sm, const int u)
+{
+    dft<16, true>(v);
+    if constexpr (Plan<L>::HAS_EXCHANGE) {
+        cplx *b = sm + 17 * u;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) b[j] = v[j];
+    }
+}
+
+// `trailing`: issue a barrier after the last shared-memory read (needed when the line is reused).
+template <int L, class SyncT>
+__device__ __forceinline__ void inv_tail(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
+                                         const SyncT &sync, const bool trailing)
 {
     typedef Plan<L> P;
     typedef Lines<L> A;
-    constexpr int T = P::T, R1 = P::R1, T2 = P::T2, T3 = P::T3;
+    constexpr int R1 = P::R1, M = P::M;
     const A a(sm, u);
     if constexpr (P::N16 == 2) {
-        dft<16, true>(v);
-#pragma unroll
-        for (int j = 0; j < 16; ++j) a.blk[j] = v[j];
-        cta_sync();
 #pragma unroll
         for (int k = 0; k < 16; ++k) v[k] = a.lin[A::link(k)];
-        cta_sync();
-        const cplx *tw1 = tw + P::TW0 + (u % T3);
+        apply_powers<16, true>(v, tw.link);
+        dft<16, true>(v);
+        if constexpr (R1 > 1) {
+            sync();
 #pragma unroll
-        for (int k = 1; k < 16; ++k) v[k] = cmulc(v[k], ld_table(&tw1[k * T3]));
+            for (int j = 0; j < 16; ++j) a.mid[A::midj(j)] = v[j];
+            sync();
+        }
     }
-    dft<16, true>(v);
     if constexpr (R1 > 1) {
-        constexpr int M = 16 / R1;
-#pragma unroll
-        for (int j = 0; j < 16; ++j) a.mid[A::midj(j)] = v[j];
-        cta_sync();
 #pragma unroll
         for (int m = 0; m < M; ++m) {
             cplx x[R1];
 #pragma unroll
             for (int k = 0; k < R1; ++k) x[k] = a.lin[A::lead(k, m)];
-            const cplx *twb = tw + u + T * m;
-#pragma unroll
-            for (int k = 1; k < R1; ++k) x[k] = cmulc(x[k], ld_table(&twb[k * T2]));
+            apply_powers<R1, true>(x, tw.lead[m]);
             dft<R1, true>(x);
 #pragma unroll
             for (int j = 0; j < R1; ++j) v[m + M * j] = x[j];
         }
-        cta_sync();
     }
+    if (P::HAS_EXCHANGE && trailing) sync();
+}
+
+// ------------------------------------------------------------------ whole transforms, one thread mapping
+template <int L, class SyncT>
+__device__ __forceinline__ void fft_fwd(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
+                                        const SyncT &sync, const bool trailing)
+{
+    fwd_head<L>(v, sm, tw, u, sync);
+    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
+    fwd_last<L>(v, sm, u);
+    if (Plan<L>::HAS_EXCHANGE && trailing) sync();
+}
+
+template <int L, class SyncT>
+__device__ __forceinline__ void fft_inv(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
+                                        const SyncT &sync, const bool trailing)
+{
+    inv_first<L>(v, sm, u);
+    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
+    inv_tail<L>(v, sm, tw, u, sync, trailing);
 }
 
 }  // namespace pgk

@@ -30,8 +30,7 @@ struct Events4 { cudaEvent_t e[4]; };
 struct pg_solver {
     int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
-    int m_h = 0;       // n_phi/2 + 1 azimuthal modes
-    int m_c = 0;       // padded to a multiple of cols_per_cta(n_r)
+    int half = 0;      // H = n_phi/2: columns of the packed spectrum Z; azimuthal modes are 0..H
     size_t field = 0;  // n_r * n_phi
 
     cudaStream_t stream = nullptr;             // borrowed
@@ -41,10 +40,11 @@ struct pg_solver {
     std::vector<char> in_pending;
 
     // device memory (owned)
-    cplx *d_W = nullptr;          // [max_batch][m_c][n_r]
-    double *d_khat = nullptr;     // [m_c][2][n_r]
-    cplx *d_tw_row = nullptr, *d_rtw = nullptr, *d_itw = nullptr;
-    cplx *d_tw_col = nullptr, *d_mod = nullptr;
+    cplx *d_W = nullptr;          // Z: [max_batch][half][n_r]
+    double *d_khat = nullptr;     // [half+1][2][n_r]
+    cplx *d_root_row = nullptr;   // [half]    exp(-2 pi i b / half)
+    cplx *d_root_col = nullptr;   // [2 n_r]   exp(-2 pi i b / (2 n_r))
+    cplx *d_cphi = nullptr;       // [half+1]  i exp(-2 pi i m / n_phi)
     double *d_rs_in = nullptr, *d_rs_out = nullptr;
     double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
     double *d_sigma_own = nullptr, *d_phi_own = nullptr;   // [max_batch][n_r][n_phi], lazily allocated
@@ -102,23 +102,6 @@ cplx unit(long double turns)   // exp(-2 pi i turns)
     return make_double2((double)cosl(a), (double)(-sinl(a)));
 }
 
-// [tw0 | tw1] of pgk::Plan for a length-L transform (see fft.cuh)
-std::vector<cplx> fft_tables(int L)
-{
-    const int n16 = (L >= 256) ? 2 : 1;
-    const int R1 = L / (n16 == 2 ? 256 : 16);
-    const int T2 = L / R1, T3 = T2 / 16;
-    std::vector<cplx> t;
-    if (R1 > 1)
-        for (int k = 0; k < R1; ++k)
-            for (int b = 0; b < T2; ++b) t.push_back(unit((long double)b * k / L));
-    if (n16 == 2)
-        for (int k = 0; k < 16; ++k)
-            for (int q = 0; q < T3; ++q) t.push_back(unit((long double)q * k / T2));
-    if (t.empty()) t.push_back(make_double2(1.0, 0.0));
-    return t;
-}
-
 template <class T>
 pg_status upload(pg_solver *s, T **dst, const std::vector<T> &src)
 {
@@ -129,48 +112,50 @@ pg_status upload(pg_solver *s, T **dst, const std::vector<T> &src)
 
 // ------------------------------------------------------------------ kernel dispatch
 template <int NPHI>
-pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rscale, int n_rows,
-                          int batch, long sigma_stride, long w_stride, cudaStream_t st)
+pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const double *rscale, int n_rows,
+                          int batch, long sigma_stride, long z_stride, cudaStream_t st)
 {
     typedef pgk::RowShape<NPHI> S;
     dim3 grid(n_rows / S::ROWS, batch);
-    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, W, s->d_tw_row, s->d_rtw, rscale, n_rows,
-                                                                 sigma_stride, w_stride);
+    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_root_row, rscale, n_rows,
+                                                                 sigma_stride, z_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
 }
 
 template <int NPHI>
-pg_status launch_rows_inv(pg_solver *s, const cplx *W, double *phi, int batch, long w_stride, long phi_stride,
+pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, long z_stride, long phi_stride,
                           cudaStream_t st)
 {
     typedef pgk::RowShape<NPHI> S;
     dim3 grid(s->n_r / S::ROWS, batch);
-    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(W, phi, s->d_tw_row, s->d_itw, s->d_rs_out, s->n_r,
-                                                                 w_stride, phi_stride);
+    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_root_row, s->d_rs_out, s->n_r,
+                                                                 z_stride, phi_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
 }
 
 template <int NR>
-pg_status launch_cols(pg_solver *s, cplx *W, int batch, long w_stride, cudaStream_t st)
+pg_status launch_cols(pg_solver *s, cplx *Z, int batch, long z_stride, cudaStream_t st)
 {
     typedef pgk::ColShape<NR> S;
-    dim3 grid(s->m_c / S::C, batch);
-    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(W, s->d_khat, s->d_tw_col, s->d_mod, w_stride);
+    const int pairs = s->half / 2 + 1;
+    dim3 grid((pairs + S::PAIRS - 1) / S::PAIRS, batch);
+    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Z, s->d_khat, s->d_root_col, s->d_cphi, s->half, z_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
 }
 
 template <int NR>
-pg_status launch_khat_cols(pg_solver *s, const cplx *Wk, double scale, cudaStream_t st)
+pg_status launch_khat_cols(pg_solver *s, const cplx *ZK, double scale, cudaStream_t st)
 {
-    typedef pgk::ColShape<NR> S;
-    dim3 grid(s->m_c / S::C, 1);
-    pgk::khat_cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Wk, s->d_khat, s->d_tw_col, s->d_mod, scale, s->m_h);
+    const int threads = 2 * (NR / 16);
+    const size_t smem = 2 * (size_t)pgk::Plan<NR>::LINE * sizeof(cplx);
+    pgk::khat_cols_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, s->d_khat, s->d_root_col, s->d_cphi, scale,
+                                                                 s->half);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
@@ -194,7 +179,7 @@ pg_status prepare_cols(pg_solver *s)
     PG_CUDA(s, cudaFuncSetAttribute(pgk::cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)S::SMEM));
     PG_CUDA(s, cudaFuncSetAttribute(pgk::khat_cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)S::SMEM));
+                                    (int)(2 * pgk::Plan<NR>::LINE * sizeof(cplx))));
     return PG_OK;
 }
 
@@ -256,7 +241,7 @@ pg_status build_khat(pg_solver *s)
     double *d_kpad = nullptr;
     cplx *d_wk = nullptr;
     const size_t kpad_n = (size_t)2 * n_r * n_phi;
-    const size_t wk_n = (size_t)s->m_c * 2 * n_r;
+    const size_t wk_n = (size_t)s->half * 2 * n_r;
     PG_CUDA(s, cudaMalloc((void **)&d_kpad, kpad_n * sizeof(double)));
     cudaError_t e = cudaMalloc((void **)&d_wk, wk_n * sizeof(cplx));
     if (e != cudaSuccess) {
@@ -266,20 +251,20 @@ pg_status build_khat(pg_solver *s)
     }
     pg_status st = PG_OK;
     do {
-        if (cudaMemsetAsync(d_wk, 0, wk_n * sizeof(cplx), s->stream) != cudaSuccess) { st = PG_ERR_CUDA; break; }
         const double eta2 = s->eps * s->eps * std::sinh(s->du) * s->dphi;
         const int threads = 256;
         const long blocks = (long)((kpad_n + threads - 1) / threads);
         pgk::green_fill_kernel<<<(unsigned)blocks, threads, 0, s->stream>>>(d_kpad, n_r, n_phi, s->du, eta2);
         s->launches++;
         if (cudaGetLastError() != cudaSuccess) { st = PG_ERR_CUDA; break; }
-        // phi transform of the 2 n_r lag rows (no radial weight), transposed into Wk[m][2 n_r]
+        // packed phi transform of the 2 n_r lag rows (no radial weight), transposed into ZK[k][2 n_r]
         st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream);
         if (st != PG_OK) break;
         // -G sinh(du) dphi (cell area / r^2), and the normalisation of the unnormalised transforms:
-        // 1/(2 n_r) for the padded radial pair, 1/n_phi for the azimuthal pair (the rows_inv
-        // pre-processing builds 2 Z, and the packed complex transform has length n_phi/2).
-        const double scale = -std::sinh(s->du) * s->dphi / (2.0 * (double)n_r * (double)n_phi);
+        // 1/(2 n_r) for the padded radial pair; 1/(2 n_phi) for the azimuthal pair (cols_kernel forms
+        // 2 X on the way in and 2 Z on the way out, the packed transform has length n_phi/2);
+        // another 1/2 because khat_cols_kernel forms 2 X of the kernel itself.
+        const double scale = -std::sinh(s->du) * s->dphi / (8.0 * (double)n_r * (double)n_phi);
         st = khat_cols(s, d_wk, scale, s->stream);
         if (st != PG_OK) break;
         if (cudaStreamSynchronize(s->stream) != cudaSuccess) { st = PG_ERR_CUDA; break; }
@@ -324,7 +309,7 @@ pg_status drain_profile(pg_solver *s)
 // the three kernels of one solve of `batch` fields starting at the given pointers
 pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx *d_W, int batch)
 {
-    const long fs = (long)s->field, ws = (long)s->m_c * s->n_r;
+    const long fs = (long)s->field, ws = (long)s->half * s->n_r;
     Events4 *ev = nullptr;
     if (s->profile) {
         if (s->prof_used == kMaxProfiledCalls) {
@@ -378,8 +363,8 @@ pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int 
 void free_all(pg_solver *s)
 {
     if (!s) return;
-    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_rtw); cudaFree(s->d_itw);
-    cudaFree(s->d_tw_col); cudaFree(s->d_mod); cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
+    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_root_row); cudaFree(s->d_root_col); cudaFree(s->d_cphi);
+    cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
     cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); cudaFree(s->d_sigma_own); cudaFree(s->d_phi_own);
     if (s->h_in) cudaFreeHost(s->h_in);
     if (s->h_out) cudaFreeHost(s->h_out);
@@ -411,9 +396,7 @@ pg_status create_impl(pg_solver *s)
 
     s->du = std::log(s->r_out / s->r_in) / n_r;
     s->dphi = 2.0 * M_PI / n_phi;
-    s->m_h = n_phi / 2 + 1;
-    const int C = pgk::cols_per_cta(n_r);
-    s->m_c = (s->m_h + C - 1) / C * C;
+    s->half = n_phi / 2;
     s->field = (size_t)n_r * n_phi;
 
     // grid tables (A1, A2): geometric centres, exact sector areas in their sinh form
@@ -435,32 +418,31 @@ pg_status create_impl(pg_solver *s)
             s2[j] = (double)(sn * sn);
         }
     }
-    // FFT tables
-    const int Lr = n_phi / 2;
-    std::vector<cplx> rtw(Lr), itw(Lr), mod(n_r);
-    for (int k = 0; k < Lr; ++k) {
-        const long double a = 2.0L * kPiL * k / n_phi;
-        rtw[k] = make_double2((double)(-0.5L * sinl(a)), (double)(-0.5L * cosl(a)));   // -(i/2) exp(-i a)
-        itw[k] = make_double2((double)(-sinl(a)), (double)cosl(a));                    //  i exp(+i a)
+    // FFT tables: unit roots of the packed row transform (length H), of the padded column transform
+    // (length 2 n_r; entry 2b is the root of the n_r-point transforms, entry n the modulation of the
+    // odd-bin branch), and c_m = i exp(-2 pi i m / n_phi) of the real-transform split
+    const int H = s->half;
+    std::vector<cplx> root_row(H), root_col(2 * (size_t)n_r), cphi(H + 1);
+    for (int b = 0; b < H; ++b) root_row[b] = unit((long double)b / H);
+    for (int b = 0; b < 2 * n_r; ++b) root_col[b] = unit((long double)b / (2.0L * n_r));
+    for (int m = 0; m <= H; ++m) {
+        const long double a = 2.0L * kPiL * m / n_phi;
+        cphi[m] = make_double2((double)sinl(a), (double)cosl(a));
     }
-    for (int n = 0; n < n_r; ++n) mod[n] = unit((long double)n / (2.0L * n_r));         // exp(-i pi n / n_r)
 
     pg_status st;
-    if ((st = upload(s, &s->d_tw_row, fft_tables(Lr))) != PG_OK) return st;
-    if ((st = upload(s, &s->d_tw_col, fft_tables(n_r))) != PG_OK) return st;
-    if ((st = upload(s, &s->d_rtw, rtw)) != PG_OK) return st;
-    if ((st = upload(s, &s->d_itw, itw)) != PG_OK) return st;
-    if ((st = upload(s, &s->d_mod, mod)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_root_row, root_row)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_root_col, root_col)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_cphi, cphi)) != PG_OK) return st;
     if ((st = upload(s, &s->d_rs_in, rs_in)) != PG_OK) return st;
     if ((st = upload(s, &s->d_rs_out, rs_out)) != PG_OK) return st;
     if ((st = upload(s, &s->d_r, s->r)) != PG_OK) return st;
     if ((st = upload(s, &s->d_dA, s->dA)) != PG_OK) return st;
     if ((st = upload(s, &s->d_s2, s2)) != PG_OK) return st;
 
-    const size_t w_n = (size_t)s->max_batch * s->m_c * n_r;
+    const size_t w_n = (size_t)s->max_batch * s->half * n_r;
     PG_CUDA(s, cudaMalloc((void **)&s->d_W, w_n * sizeof(cplx)));
-    PG_CUDA(s, cudaMemset(s->d_W, 0, w_n * sizeof(cplx)));
-    PG_CUDA(s, cudaMalloc((void **)&s->d_khat, (size_t)s->m_c * 2 * n_r * sizeof(double)));
+    PG_CUDA(s, cudaMalloc((void **)&s->d_khat, (size_t)(s->half + 1) * 2 * n_r * sizeof(double)));
 
     PG_CUDA(s, cudaStreamCreateWithFlags(&s->h2d, cudaStreamNonBlocking));
     PG_CUDA(s, cudaStreamCreateWithFlags(&s->d2h, cudaStreamNonBlocking));
@@ -621,7 +603,7 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
         const double *sg = s->d_sigma + (size_t)b * s->field;
         double *dst = host_out ? s->d_phi_own + (size_t)b * s->field : phi + (size_t)b * out_field;
         if (direct) st = launch_direct(s, sg, dst, rings ? ring0 : 0, rings ? n_rings : s->n_r, 1);
-        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * s->m_c * s->n_r, 1);
+        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * s->half * s->n_r, 1);
         if (st != PG_OK) return st;
         if (host_out) {
             PG_CUDA(s, cudaEventRecord(s->ev_solved[b], s->stream));
@@ -737,8 +719,11 @@ double pg_kernel_algorithmic_bytes(const pg_solver *s, int index, int batch)
 {
     if (!s || batch < 1) return 0.0;
     const double cells = (double)s->n_r * s->n_phi;
-    const double spec = 16.0 * s->n_r * s->m_h;          // one half-spectrum, complex128
-    const double khat = 8.0 * 2.0 * s->n_r * s->m_h;     // real spectrum of the padded kernel
+    // Hermitian half-spectrum of M_h = n_phi/2 + 1 modes.  (The packed
+    // layout Z actually holds n_phi/2 columns, 0.1 % less at 2048: modes 0 and n_phi/2 are real.)
+    const double m_h = s->half + 1;
+    const double spec = 16.0 * s->n_r * m_h;          // one half-spectrum, complex128
+    const double khat = 8.0 * 2.0 * s->n_r * m_h;     // real spectrum of the padded kernel
     switch (index) {
         case 0: return batch * (8.0 * cells + spec);              // read Sigma, write W
         case 1: return batch * (2.0 * spec) + khat;               // read W, write W, read Khat once
