@@ -1,30 +1,43 @@
 // fft.cuh -- in-register / shared-memory complex128 FFT building block for sm_100a.
 //
-// A length-L transform (L = R1 * 16^n16, R1 in {1,2,4,8}, n16 in {1,2}) is carried by T = L/16
-// threads holding 16 elements each.  Every pass is a radix-R DFT done entirely in registers;
-// between passes the T threads exchange data through a padded shared-memory line
-// (pad_idx: one spare slot every 16 keeps the stride-16 reads of the last pass conflict-free
-// for 16-byte accesses, which the hardware serves a quarter-warp at a time).
+// A length-L transform is carried by T = L/16 threads holding 16 elements each.  It is split into up
+// to three passes  L = RA * RB * RC  (decimation in frequency forward, the exact transpose backward);
+// every pass is a set of radix-R DFTs done entirely in registers, and between passes the T threads
+// exchange data through ONE padded shared-memory line.  (PAPER.md:19 names "FFT operations" as the
+// GPU-resident work; the decomposition is ours.)
 //
-// Element distribution: thread u holds indices u + T*jj (jj = 0..15) on input AND on output,
-// for both directions, so global loads/stores are coalesced and the forward spectrum can be
-// consumed by the inverse transform without any reordering (PAPER.md:19 names "FFT
-// operations" as the GPU-resident work; the decomposition is ours).
+//   pass A  radix RA, GA = 16/RA DFTs per thread, over the elements  n = MA a + b   (MA = L/RA)
+//           thread u holds n = u + T jj  (jj = a GA + g, b = u + T g): coalesced global access;
+//           y[d][b] = DFT_RA(x[.][b])[d] * w_L^(b d)                   -> slot  d MA + b
+//   pass B  radix RB (three-pass plans only), IN PLACE: thread v owns the slots
+//           { da MA + a' RC + b' : a' < RB },  b' = v mod RC,  da = v / RC (+ T/RC per extra DFT);
+//           z[da][db][b'] = DFT_RB(y[da][. RC + b'])[db] * w_MA^(b' db)  -> slot  da MA + db RC + b'
+//   pass C  radix RC on RC consecutive slots ("block" q' = da RB + db):
+//           X[q + (L/RC) c] = DFT_RC(z[da][db][.])[c],   q = da + RA db
+// Because pass B is in place, a barrier is needed only between passes (two per transform), and the
+// spectrum comes out in a fixed, plan-defined order: block q' holds the bins  q(q') + (L/RC) c.
 //
-// Twiddles.  The first version of this file read every inter-pass twiddle from a global table
-// (29 16-byte loads per thread and transform at L = 2048).  ncu showed the L1TEX data pipe as the
-// busiest unit of all three kernels with ~40 % of its wavefronts spent on those table reads, and
-// their L1/L2 latency exposed once per pass (profiles/r1_01_baseline.md).  Now a thread loads only
-// its BASE roots once (Twid<L>: w_L^(u + T m) for the leading pass, w_T2^t for the radix-16 link)
-// from one unit-root table  root[b * rs] = exp(-2 pi i b / L)  built on the host in long double,
-// and forms the powers it needs by two interleaved multiplication chains (step p^2), which costs
-// ~16 % more FP64 instructions but no table traffic.  Chains are at most 7 products deep: the
-// twiddle error stays below ~10 ulp, far inside the 1e-10 parity bar.
+// Two plan kinds:
+//   COL  RC = 16, one block per thread in pass C.  The consumer (spectral multiply by a table that
+//        is stored in the same order) never needs the natural order.
+//   ROW  RC = 8, two blocks per thread in pass C, chosen as the pair (q, L/8 - q): a thread then
+//        holds bin k together with bin L - k, which is what the real-data split ("untangle") of a
+//        packed real transform needs, so that split costs no extra exchange.
 //
-// The transform is split into a HEAD (everything up to the stores of the last exchange) and a
-// LAST pass (16 consecutive slots -> radix-16), so that a kernel may hand the last pass to a
-// different thread than the one that ran the head (rows kernels: row-fastest mapping for a
-// coalesced transposed store without an extra shared-memory transposition).
+// ODD variant of pass A (COL plans): computes the odd-frequency transform
+//        X[k] = sum_n x[n] exp(-2 pi i n (2k+1) / 2L)
+// i.e. the odd bins of the 2L-point transform of x zero-padded to 2L, by rotating the inputs of each
+// radix-RA DFT by exp(-i pi a / RA) (compile-time constants) and using odd powers of the inter-pass
+// twiddle.  No modulation table, no extra multiplies.
+//
+// Twiddles: a thread loads only BASE roots (one per DFT of pass A, one for pass B) from small
+// compact tables built on the host in long double, and forms the powers it needs by two interleaved
+// multiplication chains.  Chains are at most 8 products deep: the twiddle error stays below ~10 ulp,
+// far inside the 1e-10 parity bar.
+//
+// Shared-memory padding: slot p lives at p + p/RC, i.e. one spare slot per block, so that the block
+// stride is odd (conflict-free 16-byte accesses in pass C, which the hardware serves a quarter-warp
+// at a time) while runs of RC consecutive slots stay contiguous (passes A and B).
 #pragma once
 #include <cuda_runtime.h>
 
@@ -50,57 +63,45 @@ __device__ __forceinline__ cplx csq(cplx w)
     const double t = w.x * w.y;
     return make_double2(fma(w.x, w.x, -(w.y * w.y)), t + t);
 }
-// acc + a * w
-__device__ __forceinline__ cplx cfma(cplx a, cplx w, cplx acc)
-{
-    return make_double2(fma(-a.y, w.y, fma(a.x, w.x, acc.x)), fma(a.y, w.x, fma(a.x, w.y, acc.y)));
-}
-// acc + conj(a) * w
-__device__ __forceinline__ cplx cfmac(cplx a, cplx w, cplx acc)
-{
-    return make_double2(fma(a.y, w.y, fma(a.x, w.x, acc.x)), fma(-a.y, w.x, fma(a.x, w.y, acc.y)));
-}
 __device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
 
-__host__ __device__ constexpr int pad_idx(int a) { return a + (a >> 4); }
-
-// ------------------------------------------------------------------ compile-time twiddles
-// cos / sin of 2 pi n / 16, n = 0..7
-__host__ __device__ constexpr double cos16(int n)
+// ------------------------------------------------------------------ compile-time roots of unity
+// cos / sin of 2 pi n / 32 for any integer n
+__host__ __device__ constexpr double cos32q(int n)   // 0 <= n <= 8
 {
     return n == 0 ? 1.0
-         : n == 1 ? 0.92387953251128673848
-         : n == 2 ? 0.70710678118654752440
-         : n == 3 ? 0.38268343236508977173
-         : n == 4 ? 0.0
-         : n == 5 ? -0.38268343236508977173
-         : n == 6 ? -0.70710678118654752440
-         :          -0.92387953251128673848;
+         : n == 1 ? 0.9807852804032304491262
+         : n == 2 ? 0.9238795325112867561282
+         : n == 3 ? 0.8314696123025452370788
+         : n == 4 ? 0.7071067811865475244008
+         : n == 5 ? 0.5555702330196022247428
+         : n == 6 ? 0.3826834323650897717285
+         : n == 7 ? 0.1950903220161282678483
+         :          0.0;
 }
-__host__ __device__ constexpr double sin16(int n)
+__host__ __device__ constexpr double cos32(int n)
 {
-    return n == 0 ? 0.0
-         : n == 1 ? 0.38268343236508977173
-         : n == 2 ? 0.70710678118654752440
-         : n == 3 ? 0.92387953251128673848
-         : n == 4 ? 1.0
-         : n == 5 ? 0.92387953251128673848
-         : n == 6 ? 0.70710678118654752440
-         :          0.38268343236508977173;
+    n = ((n % 32) + 32) % 32;
+    return n <= 8 ? cos32q(n) : n <= 16 ? -cos32q(16 - n) : n <= 24 ? -cos32q(n - 16) : cos32q(32 - n);
 }
+__host__ __device__ constexpr double sin32(int n) { return cos32(n - 8); }
 
-// z * exp(-/+ 2 pi i J / N)   (- forward, + inverse), 0 <= J < N/2, N in {2,4,8,16}
-template <int J, int N, bool INV>
-__device__ __forceinline__ cplx mulw(cplx z)
+// z * exp(-/+ 2 pi i NUM / 32)   (- forward, + inverse)
+template <int NUM, bool INV>
+__device__ __forceinline__ cplx mulroot(cplx z)
 {
-    constexpr int n16 = J * (16 / N);
-    if constexpr (n16 == 0) {
+    constexpr int n = ((NUM % 32) + 32) % 32;
+    if constexpr (n == 0) {
         return z;
-    } else if constexpr (n16 == 4) {
+    } else if constexpr (n == 8) {
         return INV ? make_double2(-z.y, z.x) : make_double2(z.y, -z.x);
+    } else if constexpr (n == 16) {
+        return make_double2(-z.x, -z.y);
+    } else if constexpr (n == 24) {
+        return INV ? make_double2(z.y, -z.x) : make_double2(-z.y, z.x);
     } else {
-        constexpr double c = cos16(n16);
-        constexpr double s = INV ? sin16(n16) : -sin16(n16);   // w = c + i s
+        constexpr double c = cos32(n);
+        constexpr double s = INV ? sin32(n) : -sin32(n);   // w = c + i s
         return make_double2(fma(-z.y, s, z.x * c), fma(z.y, c, z.x * s));
     }
 }
@@ -114,7 +115,7 @@ struct DifStage {
         if constexpr (J < N / 2) {
             const cplx a = x[J], b = x[J + N / 2];
             x[J] = cadd(a, b);
-            x[J + N / 2] = mulw<J, N, INV>(csub(a, b));
+            x[J + N / 2] = mulroot<J * (32 / N), INV>(csub(a, b));
             DifStage<N, INV, J + 1>::run(x);
         }
     }
@@ -140,34 +141,61 @@ __host__ __device__ constexpr int bitrev(int k)
     return r;
 }
 
-// natural order in -> natural order out
+// natural order in -> natural order out (x is any array of at least N elements)
 template <int N, bool INV>
-__device__ __forceinline__ void dft(cplx (&x)[N])
+__device__ __forceinline__ void dft(cplx *x)
 {
-    Dif<N, INV>::run(x);
-    cplx y[N];
+    if constexpr (N >= 2) {
+        Dif<N, INV>::run(x);
+        cplx y[N];
 #pragma unroll
-    for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
+        for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
 #pragma unroll
-    for (int k = 0; k < N; ++k) x[k] = y[k];
+        for (int k = 0; k < N; ++k) x[k] = y[k];
+    }
+}
+
+// x[a] *= exp(-/+ i pi a / N), a < N  (the input rotation of the ODD transform; INV: the conjugate)
+template <int N, bool INV, int A = 1>
+__device__ __forceinline__ void rotate_half(cplx *x)
+{
+    if constexpr (A < N) {
+        x[A] = mulroot<A * (16 / N), INV>(x[A]);
+        rotate_half<N, INV, A + 1>(x);
+    }
 }
 
 // ------------------------------------------------------------------ plan
-template <int L>
+enum { COL = 0, ROW = 1 };
+
+template <int L, int KIND>
 struct Plan {
-    static_assert(L == 16 || L == 32 || L == 64 || L == 128 || L == 256 || L == 512 || L == 1024 ||
-                      L == 2048,
-                  "unsupported FFT length");
-    static constexpr int T = L / 16;                         // threads per transform
-    static constexpr int N16 = (L >= 256) ? 2 : 1;           // number of radix-16 passes
-    static constexpr int R1 = L / (N16 == 2 ? 256 : 16);     // leading small radix (1 = absent)
-    static constexpr int M = 16 / R1;                        // butterflies per thread in the leading pass
-    static constexpr int T2 = L / R1;                        // sub-length after the leading pass
-    static constexpr int T3 = T2 / 16;                       // sub-length after the first radix-16 pass
-    static constexpr int NLEAD = (R1 > 1) ? M : 1;           // base roots held for the leading pass
-    static constexpr int LINE = pad_idx(L) + 8;              // smem slots per transform (>= pad_idx(L)+1)
-    static constexpr bool HAS_EXCHANGE = (L > 16);           // false: the whole transform is one radix-16
+    static constexpr int RC = (KIND == ROW) ? 8 : 16;
+    static_assert(L >= 16 && L <= 2048 && (L & (L - 1)) == 0, "unsupported FFT length");
+    static constexpr int REST = L / RC;                                  // RA * RB
+    static constexpr int NPASS = REST == 1 ? 1 : (REST <= 16 ? 2 : 3);
+    static constexpr int RB = NPASS == 3 ? RC : 1;
+    static constexpr int RA = REST / RB;
+    static constexpr int T = L / 16;                 // threads per transform
+    static constexpr int GA = 16 / RA;               // DFTs per thread in pass A
+    static constexpr int GB = 16 / RB;               // DFTs per thread in pass B (three-pass plans)
+    static constexpr int GC = 16 / RC;               // blocks per thread in pass C
+    static constexpr int MA = L / RA;                // sub-length after pass A
+    static constexpr int NB = L / RC;                // number of blocks = stride of the bins of a block
+    static constexpr int LINE = L + L / RC;          // padded slots per transform
+    // compact twiddle table of a transform (host: polargrav.cu fills it in this order)
+    static constexpr int TW_A = 0;                   // [MA]  exp(-2 pi i b / L)
+    static constexpr int TW_AODD = MA;               // [MA]  exp(-2 pi i b / 2L)          (COL only)
+    static constexpr int TW_B = (KIND == COL) ? 2 * MA : MA;   // [RC]  exp(-2 pi i b' / MA)
+    static constexpr int TW_UN = TW_B + RC;          // [NB]  i exp(-2 pi i q / 2L)         (ROW only)
+    static constexpr int TW_LEN = TW_UN + ((KIND == ROW) ? NB : 0);
+    static_assert(NPASS < 3 || T % RC == 0, "pass B mapping needs T to be a multiple of RC");
+    // first bin of block q'
+    static __host__ __device__ constexpr int bin0(int qp) { return NPASS == 3 ? (qp / RB) + RA * (qp % RB) : qp; }
 };
+
+template <int RC>
+__host__ __device__ constexpr int pad(int p) { return p + p / RC; }
 
 // ------------------------------------------------------------------ barriers
 // Sync<T, CTA>: barrier among the T threads of one transform.  When a transform is made of whole
@@ -176,9 +204,9 @@ struct Plan {
 // otherwise the CTA-wide barrier is used (every thread of the CTA then runs the same sequence).
 template <int T, int CTA_THREADS>
 struct Sync {
-    static constexpr bool NAMED = (T >= 32) && (T < CTA_THREADS) && (CTA_THREADS / T <= 15);
+    static constexpr bool NAMED = (T >= 32) && (T < CTA_THREADS);
     int id;
-    __device__ __forceinline__ explicit Sync(int group) : id(group + 1) {}
+    __device__ __forceinline__ explicit Sync(int barrier_id) : id(barrier_id) {}
     __device__ __forceinline__ void operator()() const
     {
         if constexpr (NAMED) asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(T) : "memory");
@@ -186,200 +214,224 @@ struct Sync {
     }
 };
 
-// ------------------------------------------------------------------ shared-memory addressing
-// Every exchange address is written as (per-thread base) + (compile-time constant), so that the
-// forward and the inverse transform of one kernel share three base registers instead of keeping
-// dozens of computed addresses alive.
-//   pad_idx(a + c) = pad_idx(a) + c + c/16            when c is a multiple of 16
-//   pad_idx(16 a + j) = 17 a + j                      for 0 <= j < 16
-template <int L>
-struct Lines {
-    typedef Plan<L> P;
-    cplx *lin;   // sm + pad_idx(u)            consecutive-lane side of the radix-16 exchanges
-    cplx *mid;   // sm + pad_idx(q T2 + t)     strided side of the leading-pass exchange
-    __device__ __forceinline__ Lines(cplx *sm, int u)
-    {
-        lin = sm + (P::N16 == 2 ? pad_idx(u) : u);
-        mid = (P::N16 == 2) ? sm + (u / P::T3) * pad_idx(P::T2) + (u % P::T3) : sm + 17 * u;
-    }
-    // 16 consecutive slots of the last radix-16 pass of thread u
-    static __device__ __forceinline__ cplx *blk(cplx *sm, int u) { return sm + 17 * u; }
-    // leading pass, element (k, b = u + T m):  pad_idx(k T2 + b)
-    static __host__ __device__ constexpr int lead(int k, int m)
-    {
-        return (P::N16 == 2) ? k * pad_idx(P::T2) + pad_idx(P::T * m) : 17 * k + P::T * m;
-    }
-    // first radix-16 pass after a leading pass reads  pad_idx(q T2 + t + T3 j)
-    static __host__ __device__ constexpr int midj(int j) { return (P::N16 == 2) ? 17 * j : j; }
-    // exchange between the two radix-16 passes writes  pad_idx(u + T k)
-    static __host__ __device__ constexpr int link(int k) { return pad_idx(P::T * k); }
-};
-
-// ------------------------------------------------------------------ twiddle bases and powers
-// root[b * rs] = exp(-2 pi i b / L) for 0 <= b < L  (rs = table length / L)
-template <int L>
-struct Twid {
-    typedef Plan<L> P;
-    cplx lead[P::NLEAD];   // w_L^(u + T m), m < M            (R1 > 1)
-    cplx link;             // w_T2^t = w_L^(R1 t), t = u % T3  (N16 == 2)
-    __device__ __forceinline__ void load(const cplx *__restrict__ root, const int rs, const int u)
-    {
-        if constexpr (P::R1 > 1) {
-#pragma unroll
-            for (int m = 0; m < P::M; ++m) lead[m] = __ldg(&root[(u + P::T * m) * rs]);
-        }
-        if constexpr (P::N16 == 2) link = __ldg(&root[(u % P::T3) * P::R1 * rs]);
-    }
-};
-
-// x[k] *= p^k (CONJ: conj(p)^k) for k = 1..K-1.  Two interleaved chains a = p^(odd), b = p^(even),
-// both advanced by p^2: depth K/2, three live roots.
-template <int K, bool CONJ>
-__device__ __forceinline__ void apply_powers(cplx *x, const cplx p)
+// ------------------------------------------------------------------ twiddle powers
+// EVEN: x[d] *= s^d      (CONJ: conj(s)^d),       d = 0..K-1
+// ODD : x[d] *= s^(2d+1) (CONJ: conj),            d = 0..K-1
+// Two interleaved chains advanced by the same step keep the dependency depth at K/2.
+template <int K, bool CONJ, bool ODD>
+__device__ __forceinline__ void apply_powers(cplx *x, const cplx s)
 {
     if constexpr (K >= 2) {
-        x[1] = CONJ ? cmulc(x[1], p) : cmul(x[1], p);
-        if constexpr (K > 2) {
-            const cplx p2 = csq(p);
-            cplx a = p, b = p2;
-            x[2] = CONJ ? cmulc(x[2], b) : cmul(x[2], b);
+        const cplx s2 = csq(s);
+        cplx a, b, step;
+        if constexpr (ODD) {
+            a = s;                 // s^1, s^5, ...   (even d)
+            b = cmul(s, s2);       // s^3, s^7, ...   (odd d)
+            step = csq(s2);        // s^4
+            x[0] = CONJ ? cmulc(x[0], a) : cmul(x[0], a);
+        } else {
+            a = s2;                // s^2, s^4, ...   (even d >= 2)
+            b = s;                 // s^1, s^3, ...   (odd d)
+            step = s2;
+        }
+        x[1] = CONJ ? cmulc(x[1], b) : cmul(x[1], b);
 #pragma unroll
-            for (int k = 3; k < K; k += 2) {
-                a = cmul(a, p2);
-                x[k] = CONJ ? cmulc(x[k], a) : cmul(x[k], a);
-                if (k + 1 < K) {
-                    b = cmul(b, p2);
-                    x[k + 1] = CONJ ? cmulc(x[k + 1], b) : cmul(x[k + 1], b);
-                }
+        for (int d = 2; d < K; ++d) {
+            if (d & 1) {
+                b = cmul(b, step);
+                x[d] = CONJ ? cmulc(x[d], b) : cmul(x[d], b);
+            } else {
+                if (ODD || d > 2) a = cmul(a, step);
+                x[d] = CONJ ? cmulc(x[d], a) : cmul(x[d], a);
+            }
+        }
+    } else if constexpr (ODD) {
+        x[0] = CONJ ? cmulc(x[0], s) : cmul(x[0], s);
+    }
+}
+
+// ------------------------------------------------------------------ forward passes
+// fwd_a: v[jj] = x[u + T jj]  ->  pass A, results stored to the line (nothing stored, and v left
+// holding the rotated inputs, for one-pass plans).  No barrier.
+template <int L, int KIND, bool ODD>
+__device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
+{
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
+    if constexpr (P::NPASS == 1) {
+        if constexpr (ODD) rotate_half<16, false>(v);
+    } else {
+        const cplx *tb = tw + (ODD ? P::TW_AODD : P::TW_A) + u;
+        cplx *base = line + pad<RC>(u);
+#pragma unroll
+        for (int g = 0; g < GA; ++g) {
+            cplx x[RA];
+#pragma unroll
+            for (int a = 0; a < RA; ++a) x[a] = v[a * GA + g];
+            const cplx s = __ldg(tb + T * g);
+            if constexpr (ODD) rotate_half<RA, false>(x);
+            dft<RA, false>(x);
+            apply_powers<RA, false, ODD>(x, s);
+#pragma unroll
+            for (int d = 0; d < RA; ++d) {
+                if ((T * g) % RC == 0) base[pad<RC>(d * MA + T * g)] = x[d];
+                else line[pad<RC>(d * MA + u + T * g)] = x[d];
             }
         }
     }
 }
 
-// ------------------------------------------------------------------ forward transform
-// v[jj] = x[u + T*jj]  ->  v[k] = X[u + T*k],  X[k] = sum_n x[n] exp(-2 pi i n k / L)
-//
-// fwd_head: all passes but the last, ending with the STORES of the last exchange (no barrier).
-// fwd_last: after a barrier that covers those stores, thread u' of the transform whose line is
-//           `sm` reads its 16 slots and runs the last radix-16: v[k] = X[u' + T*k].
-// For L == 16 the head is empty and fwd_last transforms the registers it is given.
-template <int L, class SyncT>
-__device__ __forceinline__ void fwd_head(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
-                                         const SyncT &sync)
+// fwd_b: pass B in place (three-pass plans; no-op otherwise).  Call after a barrier; no barrier inside.
+template <int L, int KIND>
+__device__ __forceinline__ void fwd_b(cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
 {
-    typedef Plan<L> P;
-    typedef Lines<L> A;
-    constexpr int T = P::T, R1 = P::R1, M = P::M;
-    (void)T;
-    const A a(sm, u);
-    if constexpr (R1 > 1) {
+    typedef Plan<L, KIND> P;
+    if constexpr (P::NPASS == 3) {
+        constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
+        const int bp = u % RC, da0 = u / RC;
+        cplx *base = line + pad<RC>(da0 * MA) + bp;
+        const cplx s = __ldg(tw + P::TW_B + bp);
 #pragma unroll
-        for (int m = 0; m < M; ++m) {
-            cplx x[R1];
+        for (int h = 0; h < GB; ++h) {
+            cplx x[RB];
 #pragma unroll
-            for (int j = 0; j < R1; ++j) x[j] = v[m + M * j];
-            dft<R1, false>(x);
-            apply_powers<R1, false>(x, tw.lead[m]);
+            for (int a = 0; a < RB; ++a) x[a] = base[pad<RC>((T / RC) * h * MA + a * RC)];
+            dft<RB, false>(x);
+            apply_powers<RB, false, false>(x, s);
 #pragma unroll
-            for (int k = 0; k < R1; ++k) a.lin[A::lead(k, m)] = x[k];
+            for (int d = 0; d < RB; ++d) base[pad<RC>((T / RC) * h * MA + d * RC)] = x[d];
         }
-    }
-    if constexpr (P::N16 == 2) {
-        if constexpr (R1 > 1) {
-            sync();
-#pragma unroll
-            for (int j = 0; j < 16; ++j) v[j] = a.mid[A::midj(j)];
-            sync();
-        }
-        dft<16, false>(v);
-        apply_powers<16, false>(v, tw.link);
-#pragma unroll
-        for (int k = 0; k < 16; ++k) a.lin[A::link(k)] = v[k];
     }
 }
 
+// fwd_c (COL): after a barrier, thread u reads block u and runs the last radix-16:
+// v[c] = X[bin0(u) + T c].  One-pass plans transform the registers they are given.
 template <int L>
-__device__ __forceinline__ void fwd_last(cplx (&v)[16], const cplx *__restrict__ sm, const int u)
+__device__ __forceinline__ void fwd_c_col(cplx (&v)[16], const cplx *__restrict__ line, const int u)
 {
-    if constexpr (Plan<L>::HAS_EXCHANGE) {
-        const cplx *b = sm + 17 * u;
+    if constexpr (Plan<L, COL>::NPASS > 1) {
+        const cplx *b = line + 17 * u;
 #pragma unroll
         for (int j = 0; j < 16; ++j) v[j] = b[j];
     }
     dft<16, false>(v);
 }
 
-// ------------------------------------------------------------------ inverse transform (unnormalised)
-// v[k] = X[u + T*k]  ->  v[jj] = sum_k X[k] exp(+2 pi i n k / L),  n = u + T*jj
-// Exact transpose of the forward flow graph, with conjugated twiddles.
-//
-// inv_first: radix-16 on X[u' + T*k] and the stores of the first exchange (no barrier).
-// inv_tail : after a barrier, thread u finishes the transform.
+// fwd_c (ROW): blocks b1 -> v[0..8), b2 -> v[8..16); v[c] = X[bin0(b1) + NB c], v[8+c] = X[bin0(b2) + NB c]
 template <int L>
-__device__ __forceinline__ void inv_first(cplx (&v)[16], cplx *__restrict__ sm, const int u)
+__device__ __forceinline__ void fwd_c_row(cplx (&v)[16], const cplx *__restrict__ line, const int b1, const int b2)
+{
+    const cplx *p1 = line + 9 * b1, *p2 = line + 9 * b2;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { v[j] = p1[j]; v[8 + j] = p2[j]; }
+    dft<8, false>(&v[0]);
+    dft<8, false>(&v[8]);
+}
+
+// ------------------------------------------------------------------ inverse passes (unnormalised)
+// Exact transpose of the forward flow graph with conjugated twiddles.
+template <int L>
+__device__ __forceinline__ void inv_c_col(cplx (&v)[16], cplx *__restrict__ line, const int u)
 {
     dft<16, true>(v);
-    if constexpr (Plan<L>::HAS_EXCHANGE) {
-        cplx *b = sm + 17 * u;
+    if constexpr (Plan<L, COL>::NPASS > 1) {
+        cplx *b = line + 17 * u;
 #pragma unroll
         for (int j = 0; j < 16; ++j) b[j] = v[j];
     }
 }
 
-// `trailing`: issue a barrier after the last shared-memory read (needed when the line is reused).
-template <int L, class SyncT>
-__device__ __forceinline__ void inv_tail(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
-                                         const SyncT &sync, const bool trailing)
+template <int L>
+__device__ __forceinline__ void inv_c_row(cplx (&v)[16], cplx *__restrict__ line, const int b1, const int b2)
 {
-    typedef Plan<L> P;
-    typedef Lines<L> A;
-    constexpr int R1 = P::R1, M = P::M;
-    const A a(sm, u);
-    if constexpr (P::N16 == 2) {
+    dft<8, true>(&v[0]);
+    dft<8, true>(&v[8]);
+    cplx *p1 = line + 9 * b1, *p2 = line + 9 * b2;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] = a.lin[A::link(k)];
-        apply_powers<16, true>(v, tw.link);
-        dft<16, true>(v);
-        if constexpr (R1 > 1) {
-            sync();
-#pragma unroll
-            for (int j = 0; j < 16; ++j) a.mid[A::midj(j)] = v[j];
-            sync();
-        }
-    }
-    if constexpr (R1 > 1) {
-#pragma unroll
-        for (int m = 0; m < M; ++m) {
-            cplx x[R1];
-#pragma unroll
-            for (int k = 0; k < R1; ++k) x[k] = a.lin[A::lead(k, m)];
-            apply_powers<R1, true>(x, tw.lead[m]);
-            dft<R1, true>(x);
-#pragma unroll
-            for (int j = 0; j < R1; ++j) v[m + M * j] = x[j];
-        }
-    }
-    if (P::HAS_EXCHANGE && trailing) sync();
+    for (int j = 0; j < 8; ++j) { p1[j] = v[j]; p2[j] = v[8 + j]; }
 }
 
-// ------------------------------------------------------------------ whole transforms, one thread mapping
-template <int L, class SyncT>
-__device__ __forceinline__ void fft_fwd(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
-                                        const SyncT &sync, const bool trailing)
+template <int L, int KIND>
+__device__ __forceinline__ void inv_b(cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
 {
-    fwd_head<L>(v, sm, tw, u, sync);
-    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
-    fwd_last<L>(v, sm, u);
-    if (Plan<L>::HAS_EXCHANGE && trailing) sync();
+    typedef Plan<L, KIND> P;
+    if constexpr (P::NPASS == 3) {
+        constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
+        const int bp = u % RC, da0 = u / RC;
+        cplx *base = line + pad<RC>(da0 * MA) + bp;
+        const cplx s = __ldg(tw + P::TW_B + bp);
+#pragma unroll
+        for (int h = 0; h < GB; ++h) {
+            cplx x[RB];
+#pragma unroll
+            for (int d = 0; d < RB; ++d) x[d] = base[pad<RC>((T / RC) * h * MA + d * RC)];
+            apply_powers<RB, true, false>(x, s);
+            dft<RB, true>(x);
+#pragma unroll
+            for (int a = 0; a < RB; ++a) base[pad<RC>((T / RC) * h * MA + a * RC)] = x[a];
+        }
+    }
 }
 
-template <int L, class SyncT>
-__device__ __forceinline__ void fft_inv(cplx (&v)[16], cplx *__restrict__ sm, const Twid<L> &tw, const int u,
-                                        const SyncT &sync, const bool trailing)
+// inv_a: after a barrier; v[jj] = sum_k X[k] exp(+2 pi i n k / L) (ODD: exp(+2 pi i n (2k+1) / 2L)), n = u + T jj
+template <int L, int KIND, bool ODD>
+__device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
 {
-    inv_first<L>(v, sm, u);
-    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
-    inv_tail<L>(v, sm, tw, u, sync, trailing);
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
+    if constexpr (P::NPASS == 1) {
+        if constexpr (ODD) rotate_half<16, true>(v);
+    } else {
+        const cplx *tb = tw + (ODD ? P::TW_AODD : P::TW_A) + u;
+        const cplx *base = line + pad<RC>(u);
+#pragma unroll
+        for (int g = 0; g < GA; ++g) {
+            cplx x[RA];
+            const cplx s = __ldg(tb + T * g);
+#pragma unroll
+            for (int d = 0; d < RA; ++d) {
+                if ((T * g) % RC == 0) x[d] = base[pad<RC>(d * MA + T * g)];
+                else x[d] = line[pad<RC>(d * MA + u + T * g)];
+            }
+            apply_powers<RA, true, ODD>(x, s);
+            dft<RA, true>(x);
+            if constexpr (ODD) rotate_half<RA, true>(x);
+#pragma unroll
+            for (int a = 0; a < RA; ++a) v[a * GA + g] = x[a];
+        }
+    }
+}
+
+// slot of element n = u + T jj of the natural order (pass A's side of the line): thread u owns
+// these 16 slots during pass A, forward and inverse
+template <int L, int KIND>
+__device__ __forceinline__ int own_slot(const int u, const int jj)
+{
+    return pad<Plan<L, KIND>::RC>(u + Plan<L, KIND>::T * jj);
+}
+
+// ------------------------------------------------------------------ ROW plans: pass-C block pairs
+// Thread t of a transform takes the blocks (b1, b2) whose bins are mirror images:
+//   bins of b1:  k = q1 + NB c,   bins of b2:  L - k = q2 + NB (7 - c),   q2 = NB - q1.
+// One thread per transform is SPECIAL: it takes the two self-mirrored blocks, q = 0 (c <-> 8 - c,
+// with c = 0 the DC / Nyquist pair and c = 4 its own mirror) and q = NB/2 (c <-> 7 - c).
+template <int L>
+__device__ __forceinline__ void row_blocks(const int t, int &b1, int &b2, bool &special)
+{
+    typedef Plan<L, ROW> P;
+    if constexpr (P::NPASS == 3) {
+        constexpr int NREG = P::T - P::RB / 2;
+        if (t < NREG) { b1 = P::RB + t; b2 = P::NB - 1 - t; special = false; }
+        else {
+            const int s = t - NREG;
+            special = (s == 0);
+            b1 = s; b2 = P::RB - s;
+            if (special) b2 = P::RB / 2;
+        }
+    } else {
+        special = (t == 0);
+        b1 = t; b2 = special ? P::RA / 2 : P::RA - t;
+    }
 }
 
 }  // namespace pgk

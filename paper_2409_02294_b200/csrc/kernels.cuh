@@ -2,47 +2,49 @@
 //
 // Data layout in HBM (all fp64 / complex128), H = n_phi/2:
 //   Sigma, Phi : [B][n_r][n_phi]          phi fastest (user arrays)
-//   Z          : [B][H][n_r]   complex    TRANSPOSED packed spectrum.  Row i of Sigma (times r_i^{3/2})
-//                                         is packed as z[n] = s[2n] + i s[2n+1] and transformed with a
-//                                         complex FFT of length H; Z[k][i] is bin k of row i, so that
-//                                         column k is contiguous in r.  The Hermitian half-spectrum of
-//                                         the real row (modes 0..H) is an elementwise function of the
-//                                         column pair (k, H-k); it is formed inside the column kernel.
+//   W          : [B][H+1][n_r] complex    TRANSPOSED Hermitian half-spectrum: W[m][i] = 2 x (azimuthal mode m
+//                                         of row i of Sigma r^{3/2}), m = 0..H; column m is contiguous in r.
+//                                         Row i is packed as z[n] = s[2n] + i s[2n+1], transformed with a
+//                                         complex FFT of length H, and split into the modes of the real row
+//                                         inside the last pass of the row kernel (fft.cuh, ROW plans).
+//                                         The column kernel transforms W in place; the inverse row kernel
+//                                         re-packs and transforms back.
 //   Khat       : [H+1][2][n_r] real       spectrum of the Green's kernel for azimuthal mode m, split into
 //                                         the even (2k) and odd (2k+1) bins of the 2 n_r-point padded
-//                                         radial transform; all normalisations folded in
-//   root_row   : [H]      exp(-2 pi i b / H)            root_col : [2 n_r]  exp(-2 pi i b / (2 n_r))
-//   cphi       : [H+1]    i exp(-2 pi i m / n_phi)      (long double on the host)
+//                                         radial transform, STORED IN THE ORDER THE COLUMN KERNEL HOLDS THEM
+//                                         (entry c T + u is bin  bin0(u) + T c); all normalisations folded in
+//   tw_row, tw_col : compact twiddle tables (Plan<L,KIND>::TW_*), long double on the host
 #pragma once
 #include "fft.cuh"
 
 namespace pgk {
 
 // ---------------------------------------------------------------- shapes
-// rows per CTA in the phi passes: Z is written/read in runs of ROWS*16 bytes
+// rows per CTA in the phi passes: W is written/read in runs of ROWS*16 bytes
 __host__ __device__ constexpr int rows_per_cta(int nphi)
 {
     const int T = nphi / 32;
     const int r = 256 / (T > 0 ? T : 1);
     return r < 4 ? 4 : (r > 16 ? 16 : r);
 }
-// column pairs (k, H-k) per CTA in the r pass
-__host__ __device__ constexpr int pairs_per_cta(int nr)
+// azimuthal modes per CTA in the r pass
+__host__ __device__ constexpr int modes_per_cta(int nr)
 {
     const int T = nr / 16;
-    const int c = 64 / T;
+    const int c = 128 / T;
     return c < 1 ? 1 : (c > 8 ? 8 : c);
 }
 // Shared-memory slots between the lines of two rows of a CTA.  In the row-fastest pass a
-// quarter-warp touches (8 rows) or (4 rows x 2 neighbouring 17-slot blocks): STRIDE = 1 (mod 8)
+// quarter-warp touches (8 rows) or (4 rows x 2 neighbouring 9-slot blocks): STRIDE = 1 (mod 8)
 // resp. 2 (mod 8) spreads them over the eight 16-byte bank groups.
 template <int NPHI>
 struct RowShape {
     static constexpr int L = NPHI / 2;
-    static constexpr int T = L / 16;
+    typedef Plan<L, ROW> P;
+    static constexpr int T = P::T;
     static constexpr int ROWS = rows_per_cta(NPHI);
     static constexpr int SKEW = (ROWS >= 8) ? 1 : (8 / ROWS);
-    static constexpr int STRIDE = ((pad_idx(L) + 1 + 7) / 8) * 8 + SKEW;   // slots per row line
+    static constexpr int STRIDE = ((P::LINE + 7) / 8) * 8 + SKEW;   // slots per row line
     static constexpr int THREADS = ROWS * T;
     static constexpr size_t SMEM = (size_t)ROWS * STRIDE * sizeof(cplx);
     static constexpr int MIN_CTAS = (THREADS <= 256) ? 2 : 1;
@@ -50,48 +52,128 @@ struct RowShape {
 template <int NR>
 struct ColShape {
     static constexpr int L = NR;
-    static constexpr int T = L / 16;
-    static constexpr int PAIRS = pairs_per_cta(NR);
-    static constexpr int GROUPS = 4 * PAIRS;                // (pair, column of the pair, branch)
-    static constexpr int STRIDE = Plan<L>::LINE;
+    typedef Plan<L, COL> P;
+    static constexpr int T = P::T;
+    static constexpr int MODES = modes_per_cta(NR);
+    static constexpr int GROUPS = 2 * MODES;                // (mode, branch)
+    static constexpr int STRIDE = P::LINE;
     static constexpr int THREADS = GROUPS * T;
     static constexpr size_t SMEM = (size_t)GROUPS * STRIDE * sizeof(cplx);
-    static constexpr int MIN_CTAS = (THREADS <= 256) ? 2 : 1;   // cap registers at 128/thread
+    static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : 512 / THREADS;   // cap registers at 128/thread
 };
 
 __device__ __forceinline__ void prefetch_l1(const void *p)
 {
     asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
-// Coherent loads: unlike ld.global.nc they cannot be hoisted across a barrier by ptxas, which
-// keeps them (and the registers they occupy) where they are written.
-__device__ __forceinline__ double ld_f64(const double *p)
+__device__ __forceinline__ void named_barrier(const int id, const int threads)
 {
-    double r;
-    asm volatile("ld.global.f64 %0, [%1];" : "=d"(r) : "l"(p));
-    return r;
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
-__device__ __forceinline__ cplx ld_c128(const cplx *p)
+
+// ---------------------------------------------------------------- real-data split of the packed transform
+// (A, B) = (Z[k], Z[H-k]) of the packed transform of a real row, ck = i exp(-2 pi i k / n_phi)
+// = un * w16^C with un = i exp(-2 pi i q / n_phi) the thread's base and k = q + (H/8) C:
+//   2 X[k]   = S - ck D,          S = A + conj(B),  D = A - conj(B)
+//   2 X[H-k] = conj(S + ck D)
+template <int C>
+__device__ __forceinline__ void untangle(const cplx A, const cplx B, const cplx un, cplx &Xk, cplx &Xm)
 {
-    cplx r;
-    asm volatile("ld.global.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
-    return r;
+    const cplx S = make_double2(A.x + B.x, A.y - B.y);
+    const cplx D = make_double2(A.x - B.x, A.y + B.y);
+    const cplx P = cmul(mulroot<2 * C, false>(D), un);
+    Xk = make_double2(S.x - P.x, S.y - P.y);
+    Xm = make_double2(S.x + P.x, -(S.y + P.y));
+}
+// inverse: (Yk, Ym) = (Y[k], Y[H-k]) of the Hermitian half-spectrum  ->  packed (Z'[k], Z'[H-k]):
+//   Z'[k] = S + Q,  Z'[H-k] = conj(S - Q),   S = Yk + conj(Ym),  Q = -conj(ck) (Yk - conj(Ym))
+template <int C>
+__device__ __forceinline__ void retangle(const cplx Yk, const cplx Ym, const cplx un, cplx &Zk, cplx &Zm)
+{
+    const cplx S = make_double2(Yk.x + Ym.x, Yk.y - Ym.y);
+    const cplx D = make_double2(Yk.x - Ym.x, Yk.y + Ym.y);
+    const cplx Q = mulroot<2 * C, true>(cmulc(D, un));      // conj(ck) D
+    Zk = make_double2(S.x - Q.x, S.y - Q.y);
+    Zm = make_double2(S.x + Q.x, -(S.y + Q.y));
+}
+
+// Pass C of the ROW plan plus the split, for the regular thread (blocks b1 | b2 mirror each other)
+// and the special thread (blocks 0 and NB/2 mirror themselves).  STORE(k, value) consumes mode k.
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void split_regular(const cplx (&v)[16], const cplx un, const int q1, F &&store)
+{
+    if constexpr (C < 8) {
+        constexpr int NB = Plan<L, ROW>::NB;
+        cplx xk, xm;
+        untangle<C>(v[C], v[15 - C], un, xk, xm);
+        store(q1 + NB * C, xk);
+        store(L - q1 - NB * C, xm);
+        split_regular<L, C + 1>(v, un, q1, store);
+    }
+}
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void split_special(const cplx (&v)[16], const cplx un0, const cplx unh, F &&store)
+{
+    constexpr int NB = Plan<L, ROW>::NB;
+    if constexpr (C < 5) {          // block 0: bins NB c, mirror NB (8 - c); c = 0 is the DC / Nyquist pair
+        cplx xk, xm;
+        untangle<C>(v[C], v[(8 - C) % 8], un0, xk, xm);
+        store(NB * C, xk);
+        if (C < 4) store(L - NB * C, xm);
+        split_special<L, C + 1>(v, un0, unh, store);
+    } else if constexpr (C < 9) {   // block NB/2: bins NB/2 + NB c, mirror c <-> 7 - c
+        constexpr int c = C - 5;
+        cplx xk, xm;
+        untangle<c>(v[8 + c], v[15 - c], unh, xk, xm);
+        store(NB / 2 + NB * c, xk);
+        store(L - NB / 2 - NB * c, xm);
+        split_special<L, C + 1>(v, un0, unh, store);
+    }
+}
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void merge_regular(cplx (&v)[16], const cplx un, const int q1, F &&load)
+{
+    if constexpr (C < 8) {
+        constexpr int NB = Plan<L, ROW>::NB;
+        const cplx yk = load(q1 + NB * C), ym = load(L - q1 - NB * C);
+        retangle<C>(yk, ym, un, v[C], v[15 - C]);
+        merge_regular<L, C + 1>(v, un, q1, load);
+    }
+}
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void merge_special(cplx (&v)[16], const cplx un0, const cplx unh, F &&load)
+{
+    constexpr int NB = Plan<L, ROW>::NB;
+    if constexpr (C < 5) {
+        const cplx yk = load(NB * C), ym = load(L - NB * C);
+        cplx zk, zm;
+        retangle<C>(yk, ym, un0, zk, zm);
+        v[C] = zk;
+        if (C > 0 && C < 4) v[8 - C] = zm;
+        merge_special<L, C + 1>(v, un0, unh, load);
+    } else if constexpr (C < 9) {
+        constexpr int c = C - 5;
+        const cplx yk = load(NB / 2 + NB * c), ym = load(L - NB / 2 - NB * c);
+        retangle<c>(yk, ym, unh, v[8 + c], v[15 - c]);
+        merge_special<L, C + 1>(v, un0, unh, load);
+    }
 }
 
 // ---------------------------------------------------------------- a2: rows forward
 // One CTA transforms ROWS consecutive rows.  Row i: s = Sigma_i * scale_i (scale = r_i^{3/2}, or 1
 // when rscale == nullptr), packed as z[n] = s[2n] + i s[2n+1], complex FFT of length H = n_phi/2.
-// All passes but the last run with thread = (row, u) and u fastest (coalesced row loads); the last
-// radix-16 pass runs with thread = (u', row) and the ROW fastest, so that its outputs Z[u' + T k][i]
-// leave as runs of ROWS consecutive rows of one column: the transposed store costs no extra
-// shared-memory round trip.
+// Passes A and B run with thread = (row, u) and u fastest (coalesced row loads); pass C and the
+// real-data split run with thread = (t, row) and the ROW fastest, so that the modes W[m][i] leave as
+// runs of ROWS consecutive rows of one column: the transposed store costs no extra shared-memory
+// round trip.
 template <int NPHI>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
-rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ Z, const cplx *__restrict__ root,
+rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
                 const double *__restrict__ rscale, const int n_rows, const long sigma_field_stride,
-                const long z_field_stride)
+                const long w_field_stride)
 {
     typedef RowShape<NPHI> S;
+    typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
@@ -101,8 +183,6 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ Z, const cp
     const int i0 = blockIdx.x * ROWS;
     const int i = i0 + rho;
 
-    Twid<L> tw;
-    tw.load(root, 1, u);
     const cplx *x = reinterpret_cast<const cplx *>(sigma + blockIdx.y * sigma_field_stride + (long)i * NPHI);
     cplx v[16];
 #pragma unroll
@@ -112,28 +192,42 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ Z, const cp
 #pragma unroll
         for (int jj = 0; jj < 16; ++jj) { v[jj].x *= sc; v[jj].y *= sc; }
     }
-    const Sync<T, S::THREADS> sync(rho);
-    fwd_head<L>(v, smem + rho * S::STRIDE, tw, u, sync);
+    cplx *line = smem + rho * S::STRIDE;
+    fwd_a<L, ROW, false>(v, line, tw, u);
+    if constexpr (P::NPASS == 3) {
+        const Sync<T, S::THREADS> sync(rho + 1);
+        sync();
+        fwd_b<L, ROW>(line, tw, u);
+    }
     __syncthreads();
 
-    const int rp = tid % ROWS, up = tid / ROWS;
-    fwd_last<L>(v, smem + rp * S::STRIDE, up);
-    cplx *Zf = Z + blockIdx.y * z_field_stride + i0 + rp;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) Zf[(long)(up + T * k) * n_rows] = v[k];
+    const int rp = tid % ROWS, t = tid / ROWS;
+    int b1, b2;
+    bool special;
+    row_blocks<L>(t, b1, b2, special);
+    fwd_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
+    cplx *Wf = W + blockIdx.y * w_field_stride + i0 + rp;
+    auto store = [&](const int k, const cplx val) { Wf[(long)k * n_rows] = val; };
+    if (!special) {
+        const int q1 = P::bin0(b1);
+        split_regular<L>(v, __ldg(tw + P::TW_UN + q1), q1, store);
+    } else {
+        split_special<L>(v, __ldg(tw + P::TW_UN), __ldg(tw + P::TW_UN + P::NB / 2), store);
+    }
 }
 
 // ---------------------------------------------------------------- a4 (phi part): rows inverse
-// Reads Z'[k][i] (already rebuilt by the column kernel so that the packed inverse transform gives
-// the real row), first radix-16 pass in the row-fastest mapping (coalesced transposed load), the
-// remaining passes with u fastest, multiplies row i by oscale_i (= r_i^{-1/2}) and stores Phi_i.
+// Reads the modes W[m][i] in the row-fastest mapping (coalesced transposed load), re-packs them
+// into the spectrum of the packed row, inverse pass C; the remaining passes with u fastest;
+// multiplies row i by oscale_i (= r_i^{-1/2}) and stores Phi_i.
 template <int NPHI>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
-rows_inv_kernel(const cplx *__restrict__ Z, double *__restrict__ phi, const cplx *__restrict__ root,
-                const double *__restrict__ oscale, const int n_rows, const long z_field_stride,
+rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
+                const double *__restrict__ oscale, const int n_rows, const long w_field_stride,
                 const long phi_field_stride)
 {
     typedef RowShape<NPHI> S;
+    typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
@@ -142,19 +236,30 @@ rows_inv_kernel(const cplx *__restrict__ Z, double *__restrict__ phi, const cplx
     const int u = tid % T, rho = tid / T;
     const int i0 = blockIdx.x * ROWS;
     const int i = i0 + rho;
-    const int rp = tid % ROWS, up = tid / ROWS;
+    const int rp = tid % ROWS, t = tid / ROWS;
 
-    const cplx *Zf = Z + blockIdx.y * z_field_stride + i0 + rp;
+    int b1, b2;
+    bool special;
+    row_blocks<L>(t, b1, b2, special);
+    const cplx *Wf = W + blockIdx.y * w_field_stride + i0 + rp;
+    auto load = [&](const int k) { return Wf[(long)k * n_rows]; };
     cplx v[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) v[k] = Zf[(long)(up + T * k) * n_rows];
-    Twid<L> tw;
-    tw.load(root, 1, u);
-    inv_first<L>(v, smem + rp * S::STRIDE, up);
+    if (!special) {
+        const int q1 = P::bin0(b1);
+        merge_regular<L>(v, __ldg(tw + P::TW_UN + q1), q1, load);
+    } else {
+        merge_special<L>(v, __ldg(tw + P::TW_UN), __ldg(tw + P::TW_UN + P::NB / 2), load);
+    }
+    inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
     __syncthreads();
 
-    const Sync<T, S::THREADS> sync(rho);
-    inv_tail<L>(v, smem + rho * S::STRIDE, tw, u, sync, false);
+    cplx *line = smem + rho * S::STRIDE;
+    if constexpr (P::NPASS == 3) {
+        const Sync<T, S::THREADS> sync(rho + 1);
+        inv_b<L, ROW>(line, tw, u);
+        sync();
+    }
+    inv_a<L, ROW, false>(v, line, tw, u);
     const double sc = __ldg(&oscale[i]);
     cplx *y = reinterpret_cast<cplx *>(phi + blockIdx.y * phi_field_stride + (long)i * NPHI);
 #pragma unroll
@@ -162,129 +267,83 @@ rows_inv_kernel(const cplx *__restrict__ Z, double *__restrict__ phi, const cplx
 }
 
 // ---------------------------------------------------------------- a3 + a4 (r part): columns
-// One CTA owns PAIRS column pairs (k, H-k), k = 0..H/2.  For a pair, with A = Z[k][n], B = Z[H-k][n]
-// and c = i exp(-2 pi i k / n_phi), the two azimuthal modes of the real row transform are
-//     2 X_k     = (1 - c) A + (1 + c) conj(B)            mode k      ("a" column)
-//     2 X_{H-k} = conj( (1 + c) A + (1 - c) conj(B) )    mode H - k  ("b" column)
-// (k = 0 pairs column 0 with itself and yields modes 0 and H, the Nyquist mode; k = H/2 yields the
-// same mode twice and the "b" result is dropped).  Each mode column x[0..n_r) is convolved with the
-// Green's kernel over the radial lags, zero-padded to 2 n_r, and cropped back to n_r:
+// One CTA owns MODES azimuthal modes; mode m is the column x[0..n_r) = W[m][.].  It is convolved
+// with the Green's kernel over the radial lags, zero-padded to 2 n_r, and cropped back to n_r:
 //   y[n] = (1/2N) sum_{k'<2N} Khat[k'] Xpad[k'] e^{+2 pi i k' n / 2N},   n < N = n_r.
 // The padded 2N-point transform with a zero upper half and a cropped output is exactly two N-point
-// problems (decimation in frequency forward / in time backward):
-//   even bins: FFT_N(x)             * Khat[2k]    -> IFFT_N -> e[n]
-//   odd  bins: FFT_N(x[n] mod[n])   * Khat[2k+1]  -> IFFT_N -> o[n],   mod[n] = exp(-i pi n / N)
-//   y[n] = e[n] + conj(mod[n]) o[n]                (1/2N folded into Khat)
+// problems (decimation in frequency forward / in time backward), one per thread group ("branch"):
+//   even bins: FFT_N(x)   * Khat[2k]    -> IFFT_N    -> e[n]
+//   odd  bins: OFFT_N(x)  * Khat[2k+1]  -> IOFFT_N   -> o[n]      (odd-frequency transform, fft.cuh)
+//   y[n] = e[n] + o[n]                  (1/2N folded into Khat)
 // so the padded array and the discarded half are never formed (a3: multiply fused into the last
-// forward pass; a4: inverse with fused crop).  The four (column, branch) transforms of a pair run on
-// four thread groups with their own named barriers; they meet once, at the end, where the packed
-// spectrum of the inverse row transform is rebuilt IN PLACE:
-//     Z'[k]   = conj(1 - c) Y_k     + conj(1 + c) conj(Y_{H-k})
-//     Z'[H-k] =     (1 - c) Y_{H-k} +     (1 + c) conj(Y_k)
-template <int Q, int L, int T, int STRIDE>
-__device__ __forceinline__ void cols_combine(const cplx (&v)[16], const cplx *__restrict__ pair_lines, const int u,
-                                             const cplx alpha, const cplx beta, cplx *__restrict__ za,
-                                             cplx *__restrict__ zb, const bool store_a, const bool store_b)
-{
-#pragma unroll
-    for (int d = 0; d < 4; ++d) {
-        constexpr int dummy = 0;
-        (void)dummy;
-        const int jj = 4 * Q + d;
-        const int n = u + T * jj;
-        cplx c[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) c[q] = (q == Q) ? v[4 * Q + d] : pair_lines[q * STRIDE + n];
-        const cplx ya = cadd(c[0], c[1]);   // column a: branch 0 + branch 1
-        const cplx yb = cadd(c[2], c[3]);   // column b
-        if (store_a) {
-            cplx r = cmulc(ya, alpha);                       // conj(alpha) Y_a
-            r = cfmac(beta, cconj(yb), r);                   // + conj(beta) conj(Y_b)
-            za[n] = r;
-        }
-        if (store_b) {
-            cplx r = cmul(yb, alpha);                        // alpha Y_b
-            r = cfmac(ya, beta, r);                          // + beta conj(Y_a)
-            zb[n] = r;
-        }
-    }
-}
-
+// forward pass; a4: inverse with fused crop).  The two branches run on two thread groups with their
+// own named barriers; they meet once, at the end, where each group adds and stores half of y.
 template <int NR>
 __global__ void __launch_bounds__(ColShape<NR>::THREADS, ColShape<NR>::MIN_CTAS)
-cols_kernel(cplx *__restrict__ Z, const double *__restrict__ Khat, const cplx *__restrict__ root2,
-            const cplx *__restrict__ cphi, const int half, const long z_field_stride)
+cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw, const int n_modes,
+            const long w_field_stride)
 {
     typedef ColShape<NR> S;
+    typedef Plan<NR, COL> P;
     constexpr int L = S::L, T = S::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
 
     const int tid = threadIdx.x;
     const int u = tid % T, g = tid / T;
-    const int q = g & 3, br = g & 1, cb = (g >> 1) & 1, pl = g >> 2;
-    const int p_raw = blockIdx.x * S::PAIRS + pl;
-    const bool live = p_raw <= half / 2;
-    const int p = live ? p_raw : half / 2;
-    const int ka = p, kb = (half - p) % half;        // Z columns of the pair
-    const int mode = cb ? half - p : p;              // azimuthal mode of this group's column
+    const int br = g & 1, ml = g >> 1;
+    const int m_raw = blockIdx.x * S::MODES + ml;
+    const bool live = m_raw < n_modes;
+    const int mode = live ? m_raw : n_modes - 1;
     cplx *line = smem + g * S::STRIDE;
-    cplx *zf = Z + blockIdx.y * z_field_stride;
+    cplx *col = W + blockIdx.y * w_field_stride + (long)mode * L;
     const double *kh = Khat + ((long)mode * 2 + br) * L;
 
     // pull this group's slice of Khat into L1 while the forward transform runs
 #pragma unroll
     for (int k = 0; k < 16; ++k) prefetch_l1(kh + u + T * k);
 
-    Twid<L> tw;
-    tw.load(root2, 2, u);
-    const cplx c = __ldg(&cphi[p]);
-    const cplx alpha0 = make_double2(1.0 - c.x, -c.y), beta0 = make_double2(1.0 + c.x, c.y);
-    // this group's column: X = al P + be conj(Q)
-    const cplx al = cb ? cconj(alpha0) : alpha0, be = cb ? cconj(beta0) : beta0;
-    const cplx *P = zf + (long)(cb ? kb : ka) * L, *Qc = zf + (long)(cb ? ka : kb) * L;
-
     cplx v[16];
 #pragma unroll
-    for (int jj = 0; jj < 16; ++jj) {
-        const cplx a = P[u + T * jj], b = Qc[u + T * jj];
-        v[jj] = cfmac(b, be, cmul(a, al));
+    for (int jj = 0; jj < 16; ++jj) v[jj] = col[u + T * jj];
+
+    const Sync<T, S::THREADS> sync(g + 1);
+    if (br) fwd_a<L, COL, true>(v, line, tw, u);
+    else fwd_a<L, COL, false>(v, line, tw, u);
+    if constexpr (P::NPASS == 3) {
+        sync();
+        fwd_b<L, COL>(line, tw, u);
     }
-    if (br) {
+    if constexpr (P::NPASS > 1) sync();
+    fwd_c_col<L>(v, line, u);
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) v[jj] = cmul(v[jj], __ldg(&root2[u + T * jj]));
+    for (int k = 0; k < 16; ++k) {
+        const double kv = __ldg(kh + u + T * k);
+        v[k].x *= kv;
+        v[k].y *= kv;
     }
-    const Sync<T, S::THREADS> sync(g);
-    fwd_head<L>(v, line, tw, u, sync);
-    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
-    double kv[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) kv[k] = ld_f64(kh + u + T * k);
-    fwd_last<L>(v, line, u);
-#pragma unroll
-    for (int k = 0; k < 16; ++k) { v[k].x *= kv[k]; v[k].y *= kv[k]; }
-    // inv_first writes exactly the 16 slots this thread has just read: no barrier in between
-    inv_first<L>(v, line, u);
-    if constexpr (Plan<L>::HAS_EXCHANGE) sync();
-    inv_tail<L>(v, line, tw, u, sync, true);
-    if (br) {
-#pragma unroll
-        for (int jj = 0; jj < 16; ++jj) v[jj] = cmulc(v[jj], __ldg(&root2[u + T * jj]));
+    // inv_c writes exactly the 16 slots this thread has just read: no barrier in between
+    inv_c_col<L>(v, line, u);
+    if constexpr (P::NPASS > 1) sync();
+    if constexpr (P::NPASS == 3) {
+        inv_b<L, COL>(line, tw, u);
+        sync();
     }
-    // hand the twelve results other groups will finish to them (slot n = u + T jj of this group's line)
+    if (br) inv_a<L, COL, true>(v, line, tw, u);
+    else inv_a<L, COL, false>(v, line, tw, u);
+
+    // y = e + o: group `br` finishes elements jj in [8 br, 8 br + 8) and hands the other eight to its
+    // partner through the slots it owns (nobody else touches them after pass A)
 #pragma unroll
     for (int jj = 0; jj < 16; ++jj)
-        if ((jj >> 2) != q) line[u + T * jj] = v[jj];
-    __syncthreads();
-
-    const cplx *pair_lines = smem + (pl * 4) * S::STRIDE;
-    cplx *za = zf + (long)ka * L, *zb = zf + (long)kb * L;
-    const bool store_a = live, store_b = live && (ka != kb);
-    switch (q) {
-        case 0: cols_combine<0, L, T, S::STRIDE>(v, pair_lines, u, alpha0, beta0, za, zb, store_a, store_b); break;
-        case 1: cols_combine<1, L, T, S::STRIDE>(v, pair_lines, u, alpha0, beta0, za, zb, store_a, store_b); break;
-        case 2: cols_combine<2, L, T, S::STRIDE>(v, pair_lines, u, alpha0, beta0, za, zb, store_a, store_b); break;
-        default: cols_combine<3, L, T, S::STRIDE>(v, pair_lines, u, alpha0, beta0, za, zb, store_a, store_b); break;
+        if ((jj >> 3) != br) line[own_slot<L, COL>(u, jj)] = v[jj];
+    if constexpr (T >= 32 && 2 * T < S::THREADS) named_barrier(9 + ml, 2 * T);
+    else __syncthreads();
+    const cplx *other = smem + (g ^ 1) * S::STRIDE;
+    if (live) {
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj)
+            if ((jj >> 3) == br) col[u + T * jj] = cadd(v[jj], other[own_slot<L, COL>(u, jj)]);
     }
 }
 
@@ -308,41 +367,43 @@ __global__ void green_fill_kernel(double *__restrict__ Kpad, const int n_r, cons
     Kpad[idx] = val;
 }
 
-// Column pass of the kernel spectrum (one-time, a1).  ZK[k][0..2N) is the packed row transform of the
-// padded kernel Kpad (2N rows).  For azimuthal mode m = 0..H the mode column is rebuilt from the
-// column pair (m mod H, (H - m) mod H) exactly as in cols_kernel, then its full 2N-point forward
-// transform is taken, split into even / odd bins exactly as cols_kernel consumes them; the real
-// part is scaled and stored:  Khat[m][0][k] = scale Re X[2k],  Khat[m][1][k] = scale Re X[2k+1].
+// Column pass of the kernel spectrum (one-time, a1).  WK[m][0..2N) is azimuthal mode m of the padded
+// kernel Kpad (2N rows, from rows_fwd_kernel).  Its 2N-point forward transform is taken as the even
+// bins FFT_N(x[n] + x[n+N]) and the odd bins OFFT_N(x[n] - x[n+N]), exactly as cols_kernel consumes
+// them and in the order it holds them; the real part is scaled and stored:
+//   Khat[m][br][c T + u] = scale Re X[2 (bin0(u) + T c) + br].
 // (K is even in both lags, so X is real up to rounding.)
 template <int NR>
 __global__ void __launch_bounds__(2 * (NR / 16))
-khat_cols_kernel(const cplx *__restrict__ ZK, double *__restrict__ Khat, const cplx *__restrict__ root2,
-                 const cplx *__restrict__ cphi, const double scale, const int half)
+khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const cplx *__restrict__ tw, const double scale)
 {
-    constexpr int L = NR, T = L / 16, STRIDE = Plan<L>::LINE;
+    typedef Plan<NR, COL> P;
+    constexpr int L = NR, T = L / 16, STRIDE = P::LINE;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
 
     const int tid = threadIdx.x;
     const int u = tid % T, br = tid / T;
     const int m = blockIdx.x;                         // mode 0..H
-    const int ka = m % half, kb = (half - m) % half;
-    const cplx c = __ldg(&cphi[m]);
-    const cplx al = make_double2(1.0 - c.x, -c.y), be = make_double2(1.0 + c.x, c.y);
-    const cplx *P = ZK + (long)ka * (2 * L), *Q = ZK + (long)kb * (2 * L);
+    const cplx *col = WK + (long)m * (2 * L);
+    cplx *line = smem + br * STRIDE;
 
-    Twid<L> tw;
-    tw.load(root2, 2, u);
     cplx v[16];
 #pragma unroll
     for (int jj = 0; jj < 16; ++jj) {
         const int n = u + T * jj;
-        const cplx x1 = cfmac(Q[n], be, cmul(P[n], al));
-        const cplx x2 = cfmac(Q[n + L], be, cmul(P[n + L], al));
-        v[jj] = br ? cmul(csub(x1, x2), __ldg(&root2[n])) : cadd(x1, x2);
+        const cplx x1 = col[n], x2 = col[n + L];
+        v[jj] = br ? csub(x1, x2) : cadd(x1, x2);
     }
-    const Sync<T, 2 * T> sync(br);
-    fft_fwd<L>(v, smem + br * STRIDE, tw, u, sync, false);
+    const Sync<T, 2 * T> sync(br + 1);
+    if (br) fwd_a<L, COL, true>(v, line, tw, u);
+    else fwd_a<L, COL, false>(v, line, tw, u);
+    if constexpr (P::NPASS == 3) {
+        sync();
+        fwd_b<L, COL>(line, tw, u);
+    }
+    if constexpr (P::NPASS > 1) sync();
+    fwd_c_col<L>(v, line, u);
     double *kh = Khat + ((long)m * 2 + br) * L;
 #pragma unroll
     for (int k = 0; k < 16; ++k) kh[u + T * k] = scale * v[k].x;

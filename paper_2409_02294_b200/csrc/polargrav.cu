@@ -30,7 +30,7 @@ struct Events4 { cudaEvent_t e[4]; };
 struct pg_solver {
     int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
-    int half = 0;      // H = n_phi/2: columns of the packed spectrum Z; azimuthal modes are 0..H
+    int half = 0;      // H = n_phi/2: azimuthal modes are 0..H (H + 1 columns of W)
     size_t field = 0;  // n_r * n_phi
 
     cudaStream_t stream = nullptr;             // borrowed
@@ -40,11 +40,10 @@ struct pg_solver {
     std::vector<char> in_pending;
 
     // device memory (owned)
-    cplx *d_W = nullptr;          // Z: [max_batch][half][n_r]
+    cplx *d_W = nullptr;          // W: [max_batch][half+1][n_r]
     double *d_khat = nullptr;     // [half+1][2][n_r]
-    cplx *d_root_row = nullptr;   // [half]    exp(-2 pi i b / half)
-    cplx *d_root_col = nullptr;   // [2 n_r]   exp(-2 pi i b / (2 n_r))
-    cplx *d_cphi = nullptr;       // [half+1]  i exp(-2 pi i m / n_phi)
+    cplx *d_tw_row = nullptr;     // Plan<n_phi/2, ROW> twiddle table
+    cplx *d_tw_col = nullptr;     // Plan<n_r, COL> twiddle table
     double *d_rs_in = nullptr, *d_rs_out = nullptr;
     double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
     double *d_sigma_own = nullptr, *d_phi_own = nullptr;   // [max_batch][n_r][n_phi], lazily allocated
@@ -102,6 +101,42 @@ cplx unit(long double turns)   // exp(-2 pi i turns)
     return make_double2((double)cosl(a), (double)(-sinl(a)));
 }
 
+
+// compact twiddle table of Plan<L, KIND> (fft.cuh): base roots only, long double on the host
+template <int L, int KIND>
+void fill_twiddles(std::vector<cplx> &tw)
+{
+    typedef pgk::Plan<L, KIND> P;
+    tw.assign(P::TW_LEN, make_double2(0.0, 0.0));
+    for (int b = 0; b < P::MA; ++b) {
+        tw[P::TW_A + b] = unit((long double)b / L);
+        if (KIND == pgk::COL) tw[P::TW_AODD + b] = unit((long double)b / (2.0L * L));
+    }
+    for (int b = 0; b < P::RC; ++b) tw[P::TW_B + b] = unit((long double)b / P::MA);
+    if (KIND == pgk::ROW) {
+        for (int q = 0; q < P::NB; ++q) {       // i exp(-2 pi i q / 2L)
+            const long double a = 2.0L * kPiL * q / (2.0L * L);
+            tw[P::TW_UN + q] = make_double2((double)sinl(a), (double)cosl(a));
+        }
+    }
+}
+
+template <int KIND>
+bool twiddles_for(int len, std::vector<cplx> &tw)
+{
+    switch (len) {
+        case 16: fill_twiddles<16, KIND>(tw); return true;
+        case 32: fill_twiddles<32, KIND>(tw); return true;
+        case 64: fill_twiddles<64, KIND>(tw); return true;
+        case 128: fill_twiddles<128, KIND>(tw); return true;
+        case 256: fill_twiddles<256, KIND>(tw); return true;
+        case 512: fill_twiddles<512, KIND>(tw); return true;
+        case 1024: fill_twiddles<1024, KIND>(tw); return true;
+        case 2048: fill_twiddles<2048, KIND>(tw); return true;
+        default: return false;
+    }
+}
+
 template <class T>
 pg_status upload(pg_solver *s, T **dst, const std::vector<T> &src)
 {
@@ -117,7 +152,7 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
 {
     typedef pgk::RowShape<NPHI> S;
     dim3 grid(n_rows / S::ROWS, batch);
-    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_root_row, rscale, n_rows,
+    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_tw_row, rscale, n_rows,
                                                                  sigma_stride, z_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
@@ -130,7 +165,7 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
 {
     typedef pgk::RowShape<NPHI> S;
     dim3 grid(s->n_r / S::ROWS, batch);
-    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_root_row, s->d_rs_out, s->n_r,
+    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_tw_row, s->d_rs_out, s->n_r,
                                                                  z_stride, phi_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
@@ -141,9 +176,9 @@ template <int NR>
 pg_status launch_cols(pg_solver *s, cplx *Z, int batch, long z_stride, cudaStream_t st)
 {
     typedef pgk::ColShape<NR> S;
-    const int pairs = s->half / 2 + 1;
-    dim3 grid((pairs + S::PAIRS - 1) / S::PAIRS, batch);
-    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Z, s->d_khat, s->d_root_col, s->d_cphi, s->half, z_stride);
+    const int modes = s->half + 1;
+    dim3 grid((modes + S::MODES - 1) / S::MODES, batch);
+    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Z, s->d_khat, s->d_tw_col, modes, z_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
@@ -153,9 +188,8 @@ template <int NR>
 pg_status launch_khat_cols(pg_solver *s, const cplx *ZK, double scale, cudaStream_t st)
 {
     const int threads = 2 * (NR / 16);
-    const size_t smem = 2 * (size_t)pgk::Plan<NR>::LINE * sizeof(cplx);
-    pgk::khat_cols_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, s->d_khat, s->d_root_col, s->d_cphi, scale,
-                                                                 s->half);
+    const size_t smem = 2 * (size_t)pgk::Plan<NR, pgk::COL>::LINE * sizeof(cplx);
+    pgk::khat_cols_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, s->d_khat, s->d_tw_col, scale);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
     return PG_OK;
@@ -179,7 +213,7 @@ pg_status prepare_cols(pg_solver *s)
     PG_CUDA(s, cudaFuncSetAttribute(pgk::cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)S::SMEM));
     PG_CUDA(s, cudaFuncSetAttribute(pgk::khat_cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)(2 * pgk::Plan<NR>::LINE * sizeof(cplx))));
+                                    (int)(2 * pgk::Plan<NR, pgk::COL>::LINE * sizeof(cplx))));
     return PG_OK;
 }
 
@@ -241,7 +275,7 @@ pg_status build_khat(pg_solver *s)
     double *d_kpad = nullptr;
     cplx *d_wk = nullptr;
     const size_t kpad_n = (size_t)2 * n_r * n_phi;
-    const size_t wk_n = (size_t)s->half * 2 * n_r;
+    const size_t wk_n = (size_t)(s->half + 1) * 2 * n_r;
     PG_CUDA(s, cudaMalloc((void **)&d_kpad, kpad_n * sizeof(double)));
     cudaError_t e = cudaMalloc((void **)&d_wk, wk_n * sizeof(cplx));
     if (e != cudaSuccess) {
@@ -309,7 +343,7 @@ pg_status drain_profile(pg_solver *s)
 // the three kernels of one solve of `batch` fields starting at the given pointers
 pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx *d_W, int batch)
 {
-    const long fs = (long)s->field, ws = (long)s->half * s->n_r;
+    const long fs = (long)s->field, ws = (long)(s->half + 1) * s->n_r;
     Events4 *ev = nullptr;
     if (s->profile) {
         if (s->prof_used == kMaxProfiledCalls) {
@@ -363,7 +397,7 @@ pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int 
 void free_all(pg_solver *s)
 {
     if (!s) return;
-    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_root_row); cudaFree(s->d_root_col); cudaFree(s->d_cphi);
+    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_tw_col);
     cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
     cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); cudaFree(s->d_sigma_own); cudaFree(s->d_phi_own);
     if (s->h_in) cudaFreeHost(s->h_in);
@@ -418,29 +452,24 @@ pg_status create_impl(pg_solver *s)
             s2[j] = (double)(sn * sn);
         }
     }
-    // FFT tables: unit roots of the packed row transform (length H), of the padded column transform
-    // (length 2 n_r; entry 2b is the root of the n_r-point transforms, entry n the modulation of the
-    // odd-bin branch), and c_m = i exp(-2 pi i m / n_phi) of the real-transform split
-    const int H = s->half;
-    std::vector<cplx> root_row(H), root_col(2 * (size_t)n_r), cphi(H + 1);
-    for (int b = 0; b < H; ++b) root_row[b] = unit((long double)b / H);
-    for (int b = 0; b < 2 * n_r; ++b) root_col[b] = unit((long double)b / (2.0L * n_r));
-    for (int m = 0; m <= H; ++m) {
-        const long double a = 2.0L * kPiL * m / n_phi;
-        cphi[m] = make_double2((double)sinl(a), (double)cosl(a));
+    // FFT tables: base roots of the packed row transform (length n_phi/2) and of the n_r-point
+    // column transforms (even and odd-frequency variants), in the layout Plan<L,KIND>::TW_* expects
+    std::vector<cplx> tw_row, tw_col;
+    if (!twiddles_for<pgk::ROW>(s->half, tw_row) || !twiddles_for<pgk::COL>(n_r, tw_col)) {
+        set_err(s, "unsupported transform length");
+        return PG_ERR_UNSUPPORTED;
     }
 
     pg_status st;
-    if ((st = upload(s, &s->d_root_row, root_row)) != PG_OK) return st;
-    if ((st = upload(s, &s->d_root_col, root_col)) != PG_OK) return st;
-    if ((st = upload(s, &s->d_cphi, cphi)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_tw_row, tw_row)) != PG_OK) return st;
+    if ((st = upload(s, &s->d_tw_col, tw_col)) != PG_OK) return st;
     if ((st = upload(s, &s->d_rs_in, rs_in)) != PG_OK) return st;
     if ((st = upload(s, &s->d_rs_out, rs_out)) != PG_OK) return st;
     if ((st = upload(s, &s->d_r, s->r)) != PG_OK) return st;
     if ((st = upload(s, &s->d_dA, s->dA)) != PG_OK) return st;
     if ((st = upload(s, &s->d_s2, s2)) != PG_OK) return st;
 
-    const size_t w_n = (size_t)s->max_batch * s->half * n_r;
+    const size_t w_n = (size_t)s->max_batch * (s->half + 1) * n_r;
     PG_CUDA(s, cudaMalloc((void **)&s->d_W, w_n * sizeof(cplx)));
     PG_CUDA(s, cudaMalloc((void **)&s->d_khat, (size_t)(s->half + 1) * 2 * n_r * sizeof(double)));
 
@@ -603,7 +632,7 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
         const double *sg = s->d_sigma + (size_t)b * s->field;
         double *dst = host_out ? s->d_phi_own + (size_t)b * s->field : phi + (size_t)b * out_field;
         if (direct) st = launch_direct(s, sg, dst, rings ? ring0 : 0, rings ? n_rings : s->n_r, 1);
-        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * s->half * s->n_r, 1);
+        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * (s->half + 1) * s->n_r, 1);
         if (st != PG_OK) return st;
         if (host_out) {
             PG_CUDA(s, cudaEventRecord(s->ev_solved[b], s->stream));
@@ -719,8 +748,7 @@ double pg_kernel_algorithmic_bytes(const pg_solver *s, int index, int batch)
 {
     if (!s || batch < 1) return 0.0;
     const double cells = (double)s->n_r * s->n_phi;
-    // Hermitian half-spectrum of M_h = n_phi/2 + 1 modes.  (The packed
-    // layout Z actually holds n_phi/2 columns, 0.1 % less at 2048: modes 0 and n_phi/2 are real.)
+    // Hermitian half-spectrum of M_h = n_phi/2 + 1 modes (the columns of W)
     const double m_h = s->half + 1;
     const double spec = 16.0 * s->n_r * m_h;          // one half-spectrum, complex128
     const double khat = 8.0 * 2.0 * s->n_r * m_h;     // real spectrum of the padded kernel
