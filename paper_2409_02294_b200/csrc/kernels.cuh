@@ -58,7 +58,9 @@ struct ColShape {
     static constexpr int GROUPS = 2 * MODES;                // (mode, branch)
     static constexpr int STRIDE = P::LINE;
     static constexpr int THREADS = GROUPS * T;
-    static constexpr size_t SMEM = (size_t)GROUPS * STRIDE * sizeof(cplx);
+    static constexpr size_t LINES = (size_t)GROUPS * STRIDE * sizeof(cplx);
+    static constexpr size_t KSTAGE = (size_t)GROUPS * L * sizeof(double);   // Khat slices of the CTA's modes
+    static constexpr size_t SMEM = LINES + KSTAGE + 16;                     // + one mbarrier
     static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : 512 / THREADS;   // cap registers at 128/thread
 };
 
@@ -69,6 +71,34 @@ __device__ __forceinline__ void prefetch_l1(const void *p)
 __device__ __forceinline__ void named_barrier(const int id, const int threads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+
+// ---------------------------------------------------------------- bulk asynchronous copy (TMA, 1-D)
+// global -> shared, completion signalled on an mbarrier by transferred bytes
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, const int arrivals)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(arrivals) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_load(void *dst_smem, const void *src_global, const unsigned bytes,
+                                          unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_addr(dst_smem)),
+                 "l"(src_global), "r"(bytes), "r"(smem_addr(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, const unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done)
+                     : "r"(smem_addr(bar)), "r"(parity)
+                     : "memory");
+    } while (!done);
 }
 
 // ---------------------------------------------------------------- real-data split of the packed transform
@@ -297,11 +327,19 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     const int mode = live ? m_raw : n_modes - 1;
     cplx *line = smem + g * S::STRIDE;
     cplx *col = W + blockIdx.y * w_field_stride + (long)mode * L;
-    const double *kh = Khat + ((long)mode * 2 + br) * L;
 
-    // pull this group's slice of Khat into L1 while the forward transform runs
-#pragma unroll
-    for (int k = 0; k < 16; ++k) prefetch_l1(kh + u + T * k);
+    // the Khat slices of this CTA's modes are contiguous: one bulk asynchronous copy into shared
+    // memory, issued now and waited for after the forward transform
+    double *kstage = reinterpret_cast<double *>(smem_raw + S::LINES);
+    unsigned long long *kbar = reinterpret_cast<unsigned long long *>(smem_raw + S::LINES + S::KSTAGE);
+    if (tid == 0) mbar_init(kbar, 1);
+    __syncthreads();
+    if (tid == 0) {
+        const int m0 = blockIdx.x * S::MODES;
+        const int nm = (n_modes - m0 < S::MODES) ? n_modes - m0 : S::MODES;
+        bulk_load(kstage, Khat + (long)m0 * 2 * L, (unsigned)(nm * 2 * L * sizeof(double)), kbar);
+    }
+    const double *kh = kstage + g * L;
 
     cplx v[16];
 #pragma unroll
@@ -316,9 +354,10 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     }
     if constexpr (P::NPASS > 1) sync();
     fwd_c_col<L>(v, line, u);
+    mbar_wait(kbar, 0);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        const double kv = __ldg(kh + u + T * k);
+        const double kv = kh[u + T * k];
         v[k].x *= kv;
         v[k].y *= kv;
     }
