@@ -250,25 +250,41 @@ __device__ __forceinline__ void apply_powers(cplx *x, const cplx s)
     }
 }
 
+// ------------------------------------------------------------------ twiddle bases of one thread
+// Only the table addresses are kept; a base root is loaded where it is used (holding the roots in
+// registers across the transform costs 8-12 registers and pushes the 128-register kernels into
+// local-memory spills: measured 76 -> 97 us per solve at 2048^2).
+template <int L, int KIND>
+struct Bases {
+    typedef Plan<L, KIND> P;
+    const cplx *tw;
+    __device__ __forceinline__ void load(const cplx *__restrict__ table, const int, const bool) { tw = table; }
+    template <bool ODD>
+    __device__ __forceinline__ cplx a(const int u, const int g) const
+    {
+        return __ldg(tw + (ODD ? P::TW_AODD : P::TW_A) + u + P::T * g);
+    }
+    __device__ __forceinline__ cplx b(const int u) const { return __ldg(tw + P::TW_B + u % P::RC); }
+};
+
 // ------------------------------------------------------------------ forward passes
 // fwd_a: v[jj] = x[u + T jj]  ->  pass A, results stored to the line (nothing stored, and v left
 // holding the rotated inputs, for one-pass plans).  No barrier.
 template <int L, int KIND, bool ODD>
-__device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
+__device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
     if constexpr (P::NPASS == 1) {
         if constexpr (ODD) rotate_half<16, false>(v);
     } else {
-        const cplx *tb = tw + (ODD ? P::TW_AODD : P::TW_A) + u;
         cplx *base = line + pad<RC>(u);
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
 #pragma unroll
             for (int a = 0; a < RA; ++a) x[a] = v[a * GA + g];
-            const cplx s = __ldg(tb + T * g);
+            const cplx s = tw.template a<ODD>(u, g);
             if constexpr (ODD) rotate_half<RA, false>(x);
             dft<RA, false>(x);
             apply_powers<RA, false, ODD>(x, s);
@@ -283,14 +299,14 @@ __device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, co
 
 // fwd_b: pass B in place (three-pass plans; no-op otherwise).  Call after a barrier; no barrier inside.
 template <int L, int KIND>
-__device__ __forceinline__ void fwd_b(cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
+__device__ __forceinline__ void fwd_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     if constexpr (P::NPASS == 3) {
         constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
         const int bp = u % RC, da0 = u / RC;
         cplx *base = line + pad<RC>(da0 * MA) + bp;
-        const cplx s = __ldg(tw + P::TW_B + bp);
+        const cplx s = tw.b(u);
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
             cplx x[RB];
@@ -352,14 +368,14 @@ __device__ __forceinline__ void inv_c_row(cplx (&v)[16], cplx *__restrict__ line
 }
 
 template <int L, int KIND>
-__device__ __forceinline__ void inv_b(cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
+__device__ __forceinline__ void inv_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     if constexpr (P::NPASS == 3) {
         constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
         const int bp = u % RC, da0 = u / RC;
         cplx *base = line + pad<RC>(da0 * MA) + bp;
-        const cplx s = __ldg(tw + P::TW_B + bp);
+        const cplx s = tw.b(u);
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
             cplx x[RB];
@@ -375,19 +391,18 @@ __device__ __forceinline__ void inv_b(cplx *__restrict__ line, const cplx *__res
 
 // inv_a: after a barrier; v[jj] = sum_k X[k] exp(+2 pi i n k / L) (ODD: exp(+2 pi i n (2k+1) / 2L)), n = u + T jj
 template <int L, int KIND, bool ODD>
-__device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const cplx *__restrict__ tw, const int u)
+__device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
     if constexpr (P::NPASS == 1) {
         if constexpr (ODD) rotate_half<16, true>(v);
     } else {
-        const cplx *tb = tw + (ODD ? P::TW_AODD : P::TW_A) + u;
         const cplx *base = line + pad<RC>(u);
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
-            const cplx s = __ldg(tb + T * g);
+            const cplx s = tw.template a<ODD>(u, g);
 #pragma unroll
             for (int d = 0; d < RA; ++d) {
                 if ((T * g) % RC == 0) x[d] = base[pad<RC>(d * MA + T * g)];

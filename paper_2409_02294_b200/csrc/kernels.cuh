@@ -17,6 +17,10 @@
 #pragma once
 #include "fft.cuh"
 
+#ifndef PG_ROW_THREADS
+#define PG_ROW_THREADS 128
+#endif
+
 namespace pgk {
 
 // ---------------------------------------------------------------- shapes
@@ -24,8 +28,8 @@ namespace pgk {
 __host__ __device__ constexpr int rows_per_cta(int nphi)
 {
     const int T = nphi / 32;
-    const int r = 256 / (T > 0 ? T : 1);
-    return r < 4 ? 4 : (r > 16 ? 16 : r);
+    const int r = PG_ROW_THREADS / (T > 0 ? T : 1);
+    return r < 2 ? 2 : (r > 16 ? 16 : r);
 }
 // azimuthal modes per CTA in the r pass
 __host__ __device__ constexpr int modes_per_cta(int nr)
@@ -46,8 +50,11 @@ struct RowShape {
     static constexpr int SKEW = (ROWS >= 8) ? 1 : (8 / ROWS);
     static constexpr int STRIDE = ((P::LINE + 7) / 8) * 8 + SKEW;   // slots per row line
     static constexpr int THREADS = ROWS * T;
-    static constexpr size_t SMEM = (size_t)ROWS * STRIDE * sizeof(cplx);
-    static constexpr int MIN_CTAS = (THREADS <= 256) ? 2 : 1;
+    static constexpr int SLOTS = 17;                                // prefetch slots per thread (16 fwd, 17 inv)
+    static constexpr size_t SMEM = ((size_t)ROWS * STRIDE + (size_t)SLOTS * THREADS) * sizeof(cplx);
+    // resident CTAs per SM are set by shared memory (227 KB); registers are capped to match
+    static constexpr int BY_SMEM = (int)((227 * 1024) / (SMEM + 1024));
+    static constexpr int MIN_CTAS = BY_SMEM < 1 ? 1 : (BY_SMEM * THREADS > 512 ? (512 / THREADS > 0 ? 512 / THREADS : 1) : BY_SMEM);
 };
 template <int NR>
 struct ColShape {
@@ -61,7 +68,7 @@ struct ColShape {
     static constexpr size_t LINES = (size_t)GROUPS * STRIDE * sizeof(cplx);
     static constexpr size_t KSTAGE = (size_t)GROUPS * L * sizeof(double);   // Khat slices of the CTA's modes
     static constexpr size_t SMEM = LINES + KSTAGE + 16;                     // + one mbarrier
-    static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : 512 / THREADS;   // cap registers at 128/thread
+    static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : (THREADS <= 128 ? 4 : 512 / THREADS);   // cap registers at 128/thread
 };
 
 __device__ __forceinline__ void prefetch_l1(const void *p)
@@ -160,38 +167,86 @@ __device__ __forceinline__ void split_special(const cplx (&v)[16], const cplx un
         split_special<L, C + 1>(v, un0, unh, store);
     }
 }
+// Inverse direction.  The modes a thread needs are enumerated twice in the same order: once to
+// prefetch them (modes_*: f(slot, k)), once to consume them (merge_*: get(slot)).
+//   regular: slot 2C   = mode q1 + NB C,  slot 2C+1 = its mirror
+//   special: slots 0..8 = block 0 (0, L | NB, L-NB | 2NB, L-2NB | 3NB, L-3NB | L/2), slots 9..16 = block NB/2
 template <int L, int C = 0, class F>
-__device__ __forceinline__ void merge_regular(cplx (&v)[16], const cplx un, const int q1, F &&load)
+__device__ __forceinline__ void modes_regular(const int q1, F &&f)
 {
     if constexpr (C < 8) {
         constexpr int NB = Plan<L, ROW>::NB;
-        const cplx yk = load(q1 + NB * C), ym = load(L - q1 - NB * C);
-        retangle<C>(yk, ym, un, v[C], v[15 - C]);
-        merge_regular<L, C + 1>(v, un, q1, load);
+        f(2 * C, q1 + NB * C);
+        f(2 * C + 1, L - q1 - NB * C);
+        modes_regular<L, C + 1>(q1, f);
     }
 }
 template <int L, int C = 0, class F>
-__device__ __forceinline__ void merge_special(cplx (&v)[16], const cplx un0, const cplx unh, F &&load)
+__device__ __forceinline__ void modes_special(F &&f)
 {
     constexpr int NB = Plan<L, ROW>::NB;
-    if constexpr (C < 5) {
-        const cplx yk = load(NB * C), ym = load(L - NB * C);
-        cplx zk, zm;
-        retangle<C>(yk, ym, un0, zk, zm);
-        v[C] = zk;
-        if (C > 0 && C < 4) v[8 - C] = zm;
-        merge_special<L, C + 1>(v, un0, unh, load);
+    if constexpr (C < 4) {
+        f(2 * C, NB * C);
+        f(2 * C + 1, L - NB * C);
+        modes_special<L, C + 1>(f);
+    } else if constexpr (C == 4) {
+        f(8, L / 2);
+        modes_special<L, C + 1>(f);
     } else if constexpr (C < 9) {
         constexpr int c = C - 5;
-        const cplx yk = load(NB / 2 + NB * c), ym = load(L - NB / 2 - NB * c);
-        retangle<c>(yk, ym, unh, v[8 + c], v[15 - c]);
-        merge_special<L, C + 1>(v, un0, unh, load);
+        f(9 + 2 * c, NB / 2 + NB * c);
+        f(10 + 2 * c, L - NB / 2 - NB * c);
+        modes_special<L, C + 1>(f);
+    }
+}
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void merge_regular(cplx (&v)[16], const cplx un, F &&get)
+{
+    if constexpr (C < 8) {
+        retangle<C>(get(2 * C), get(2 * C + 1), un, v[C], v[15 - C]);
+        merge_regular<L, C + 1>(v, un, get);
+    }
+}
+template <int L, int C = 0, class F>
+__device__ __forceinline__ void merge_special(cplx (&v)[16], const cplx un0, const cplx unh, F &&get)
+{
+    if constexpr (C < 4) {
+        cplx zk, zm;
+        retangle<C>(get(2 * C), get(2 * C + 1), un0, zk, zm);
+        v[C] = zk;
+        if (C > 0) v[8 - C] = zm;
+        merge_special<L, C + 1>(v, un0, unh, get);
+    } else if constexpr (C == 4) {
+        cplx zk, zm;
+        const cplx y = get(8);
+        retangle<4>(y, y, un0, zk, zm);
+        v[4] = zk;
+        merge_special<L, C + 1>(v, un0, unh, get);
+    } else if constexpr (C < 9) {
+        constexpr int c = C - 5;
+        retangle<c>(get(9 + 2 * c), get(10 + 2 * c), unh, v[8 + c], v[15 - c]);
+        merge_special<L, C + 1>(v, un0, unh, get);
     }
 }
 
+// ---------------------------------------------------------------- per-thread asynchronous prefetch
+// cp.async (LDGSTS) global -> shared, 16 bytes, bypassing L1 and the register file.  Each thread
+// prefetches exactly the elements it will consume itself, into slots only it touches
+// (slot j of thread tid = stage[j * THREADS + tid]: conflict-free), so no barrier is involved:
+// the thread waits for its own group, moves the slots to registers and at once reuses them for
+// the next work item.
+__device__ __forceinline__ void cp_async16(void *dst_smem, const void *src_global)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr(dst_smem)), "l"(src_global) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // ---------------------------------------------------------------- a2: rows forward
-// One CTA transforms ROWS consecutive rows.  Row i: s = Sigma_i * scale_i (scale = r_i^{3/2}, or 1
-// when rscale == nullptr), packed as z[n] = s[2n] + i s[2n+1], complex FFT of length H = n_phi/2.
+// PERSISTENT: a CTA walks over work items (ROWS consecutive rows of one field), item = blockIdx.x +
+// k gridDim.x, prefetching the next item's rows with cp.async while it transforms the current one.
+// Row i: s = Sigma_i * scale_i (scale = r_i^{3/2}, or 1 when rscale == nullptr), packed as
+// z[n] = s[2n] + i s[2n+1], complex FFT of length H = n_phi/2.
 // Passes A and B run with thread = (row, u) and u fastest (coalesced row loads); pass C and the
 // real-data split run with thread = (t, row) and the ROW fastest, so that the modes W[m][i] leave as
 // runs of ROWS consecutive rows of one column: the transposed store costs no extra shared-memory
@@ -199,7 +254,7 @@ __device__ __forceinline__ void merge_special(cplx (&v)[16], const cplx un0, con
 template <int NPHI>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
-                const double *__restrict__ rscale, const int n_rows, const long sigma_field_stride,
+                const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
                 const long w_field_stride)
 {
     typedef RowShape<NPHI> S;
@@ -207,53 +262,70 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
+    cplx *stage = smem + ROWS * S::STRIDE + threadIdx.x;
 
     const int tid = threadIdx.x;
     const int u = tid % T, rho = tid / T;
-    const int i0 = blockIdx.x * ROWS;
-    const int i = i0 + rho;
-
-    const cplx *x = reinterpret_cast<const cplx *>(sigma + blockIdx.y * sigma_field_stride + (long)i * NPHI);
-    cplx v[16];
-#pragma unroll
-    for (int jj = 0; jj < 16; ++jj) v[jj] = x[u + T * jj];
-    if (rscale != nullptr) {
-        const double sc = __ldg(&rscale[i]);
-#pragma unroll
-        for (int jj = 0; jj < 16; ++jj) { v[jj].x *= sc; v[jj].y *= sc; }
-    }
-    cplx *line = smem + rho * S::STRIDE;
-    fwd_a<L, ROW, false>(v, line, tw, u);
-    if constexpr (P::NPASS == 3) {
-        const Sync<T, S::THREADS> sync(rho + 1);
-        sync();
-        fwd_b<L, ROW>(line, tw, u);
-    }
-    __syncthreads();
-
     const int rp = tid % ROWS, t = tid / ROWS;
+    const int items_per_field = n_rows / ROWS;
+    cplx *line = smem + rho * S::STRIDE;
     int b1, b2;
     bool special;
     row_blocks<L>(t, b1, b2, special);
-    fwd_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
-    cplx *Wf = W + blockIdx.y * w_field_stride + i0 + rp;
-    auto store = [&](const int k, const cplx val) { Wf[(long)k * n_rows] = val; };
-    if (!special) {
-        const int q1 = P::bin0(b1);
-        split_regular<L>(v, __ldg(tw + P::TW_UN + q1), q1, store);
-    } else {
-        split_special<L>(v, __ldg(tw + P::TW_UN), __ldg(tw + P::TW_UN + P::NB / 2), store);
+    const int q1 = P::bin0(b1);
+    const cplx un1 = __ldg(tw + P::TW_UN + (special ? 0 : q1));
+    const cplx un2 = __ldg(tw + P::TW_UN + P::NB / 2);
+    Bases<L, ROW> bases;
+    bases.load(tw, u, false);
+
+    auto prefetch = [&](const int item) {
+        const int f = item / items_per_field, i = (item % items_per_field) * ROWS + rho;
+        const cplx *x = reinterpret_cast<const cplx *>(sigma + f * sigma_field_stride + (long)i * NPHI) + u;
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj) cp_async16(stage + jj * S::THREADS, x + T * jj);
+        cp_async_commit();
+    };
+
+    int item = blockIdx.x;
+    if (item < n_items) prefetch(item);
+    for (; item < n_items; item += gridDim.x) {
+        const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
+        cplx v[16];
+        const double sc = (rscale != nullptr) ? __ldg(&rscale[i0 + rho]) : 1.0;
+        cp_async_wait_all();
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj) v[jj] = stage[jj * S::THREADS];
+        if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        if (rscale != nullptr) {
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) { v[jj].x *= sc; v[jj].y *= sc; }
+        }
+        fwd_a<L, ROW, false>(v, line, bases, u);
+        if constexpr (P::NPASS == 3) {
+            const Sync<T, S::THREADS> sync(rho + 1);
+            sync();
+            fwd_b<L, ROW>(line, bases, u);
+        }
+        __syncthreads();
+
+        fwd_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
+        cplx *Wf = W + f * w_field_stride + i0 + rp;
+        auto store = [&](const int k, const cplx val) { Wf[(long)k * n_rows] = val; };
+        if (!special) split_regular<L>(v, un1, q1, store);
+        else split_special<L>(v, un1, un2, store);
+        __syncthreads();   // the lines are rewritten by the next item's pass A
     }
 }
 
 // ---------------------------------------------------------------- a4 (phi part): rows inverse
-// Reads the modes W[m][i] in the row-fastest mapping (coalesced transposed load), re-packs them
-// into the spectrum of the packed row, inverse pass C; the remaining passes with u fastest;
-// multiplies row i by oscale_i (= r_i^{-1/2}) and stores Phi_i.
+// PERSISTENT like rows_fwd_kernel.  Prefetches the modes W[m][i] it needs in the row-fastest
+// mapping (transposed access in runs of ROWS rows), re-packs them into the spectrum of the packed
+// row, inverse pass C; the remaining passes with u fastest; multiplies row i by oscale_i
+// (= r_i^{-1/2}) and stores Phi_i.
 template <int NPHI>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
-                const double *__restrict__ oscale, const int n_rows, const long w_field_stride,
+                const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
                 const long phi_field_stride)
 {
     typedef RowShape<NPHI> S;
@@ -261,39 +333,56 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
+    cplx *stage = smem + ROWS * S::STRIDE + threadIdx.x;
 
     const int tid = threadIdx.x;
     const int u = tid % T, rho = tid / T;
-    const int i0 = blockIdx.x * ROWS;
-    const int i = i0 + rho;
     const int rp = tid % ROWS, t = tid / ROWS;
-
+    const int items_per_field = n_rows / ROWS;
+    cplx *line = smem + rho * S::STRIDE;
     int b1, b2;
     bool special;
     row_blocks<L>(t, b1, b2, special);
-    const cplx *Wf = W + blockIdx.y * w_field_stride + i0 + rp;
-    auto load = [&](const int k) { return Wf[(long)k * n_rows]; };
-    cplx v[16];
-    if (!special) {
-        const int q1 = P::bin0(b1);
-        merge_regular<L>(v, __ldg(tw + P::TW_UN + q1), q1, load);
-    } else {
-        merge_special<L>(v, __ldg(tw + P::TW_UN), __ldg(tw + P::TW_UN + P::NB / 2), load);
-    }
-    inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
-    __syncthreads();
+    const int q1 = P::bin0(b1);
+    const cplx un1 = __ldg(tw + P::TW_UN + (special ? 0 : q1));
+    const cplx un2 = __ldg(tw + P::TW_UN + P::NB / 2);
+    Bases<L, ROW> bases;
+    bases.load(tw, u, false);
 
-    cplx *line = smem + rho * S::STRIDE;
-    if constexpr (P::NPASS == 3) {
-        const Sync<T, S::THREADS> sync(rho + 1);
-        inv_b<L, ROW>(line, tw, u);
-        sync();
-    }
-    inv_a<L, ROW, false>(v, line, tw, u);
-    const double sc = __ldg(&oscale[i]);
-    cplx *y = reinterpret_cast<cplx *>(phi + blockIdx.y * phi_field_stride + (long)i * NPHI);
+    auto prefetch = [&](const int item) {
+        const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
+        const cplx *Wf = W + f * w_field_stride + i0 + rp;
+        auto fetch = [&](const int slot, const int k) { cp_async16(stage + slot * S::THREADS, Wf + (long)k * n_rows); };
+        if (!special) modes_regular<L>(q1, fetch);
+        else modes_special<L>(fetch);
+        cp_async_commit();
+    };
+    auto get = [&](const int slot) { return stage[slot * S::THREADS]; };
+
+    int item = blockIdx.x;
+    if (item < n_items) prefetch(item);
+    for (; item < n_items; item += gridDim.x) {
+        const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
+        cplx v[16];
+        const double sc = __ldg(&oscale[i0 + rho]);
+        cp_async_wait_all();
+        if (!special) merge_regular<L>(v, un1, get);
+        else merge_special<L>(v, un1, un2, get);
+        if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
+        __syncthreads();
+
+        if constexpr (P::NPASS == 3) {
+            const Sync<T, S::THREADS> sync(rho + 1);
+            inv_b<L, ROW>(line, bases, u);
+            sync();
+        }
+        inv_a<L, ROW, false>(v, line, bases, u);
+        cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * NPHI);
 #pragma unroll
-    for (int jj = 0; jj < 16; ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
+        for (int jj = 0; jj < 16; ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
+        __syncthreads();   // the lines are rewritten by the next item's pass C
+    }
 }
 
 // ---------------------------------------------------------------- a3 + a4 (r part): columns
@@ -344,13 +433,15 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     cplx v[16];
 #pragma unroll
     for (int jj = 0; jj < 16; ++jj) v[jj] = col[u + T * jj];
+    Bases<L, COL> bases;
+    bases.load(tw, u, br != 0);
 
     const Sync<T, S::THREADS> sync(g + 1);
-    if (br) fwd_a<L, COL, true>(v, line, tw, u);
-    else fwd_a<L, COL, false>(v, line, tw, u);
+    if (br) fwd_a<L, COL, true>(v, line, bases, u);
+    else fwd_a<L, COL, false>(v, line, bases, u);
     if constexpr (P::NPASS == 3) {
         sync();
-        fwd_b<L, COL>(line, tw, u);
+        fwd_b<L, COL>(line, bases, u);
     }
     if constexpr (P::NPASS > 1) sync();
     fwd_c_col<L>(v, line, u);
@@ -365,11 +456,11 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     inv_c_col<L>(v, line, u);
     if constexpr (P::NPASS > 1) sync();
     if constexpr (P::NPASS == 3) {
-        inv_b<L, COL>(line, tw, u);
+        inv_b<L, COL>(line, bases, u);
         sync();
     }
-    if (br) inv_a<L, COL, true>(v, line, tw, u);
-    else inv_a<L, COL, false>(v, line, tw, u);
+    if (br) inv_a<L, COL, true>(v, line, bases, u);
+    else inv_a<L, COL, false>(v, line, bases, u);
 
     // y = e + o: group `br` finishes elements jj in [8 br, 8 br + 8) and hands the other eight to its
     // partner through the slots it owns (nobody else touches them after pass A)
@@ -434,12 +525,14 @@ khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const c
         const cplx x1 = col[n], x2 = col[n + L];
         v[jj] = br ? csub(x1, x2) : cadd(x1, x2);
     }
+    Bases<L, COL> bases;
+    bases.load(tw, u, br != 0);
     const Sync<T, 2 * T> sync(br + 1);
-    if (br) fwd_a<L, COL, true>(v, line, tw, u);
-    else fwd_a<L, COL, false>(v, line, tw, u);
+    if (br) fwd_a<L, COL, true>(v, line, bases, u);
+    else fwd_a<L, COL, false>(v, line, bases, u);
     if constexpr (P::NPASS == 3) {
         sync();
-        fwd_b<L, COL>(line, tw, u);
+        fwd_b<L, COL>(line, bases, u);
     }
     if constexpr (P::NPASS > 1) sync();
     fwd_c_col<L>(v, line, u);

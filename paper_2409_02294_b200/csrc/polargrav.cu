@@ -30,6 +30,7 @@ struct Events4 { cudaEvent_t e[4]; };
 struct pg_solver {
     int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
+    int sm_count = 0, row_ctas = 0;   // persistent grid of the row kernels
     int half = 0;      // H = n_phi/2: azimuthal modes are 0..H (H + 1 columns of W)
     size_t field = 0;  // n_r * n_phi
 
@@ -151,8 +152,9 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
                           int batch, long sigma_stride, long z_stride, cudaStream_t st)
 {
     typedef pgk::RowShape<NPHI> S;
-    dim3 grid(n_rows / S::ROWS, batch);
-    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_tw_row, rscale, n_rows,
+    const int n_items = (n_rows / S::ROWS) * batch;      // persistent CTAs walk over the items
+    const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
+    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_tw_row, rscale, n_rows, n_items,
                                                                  sigma_stride, z_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
@@ -164,8 +166,9 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
                           cudaStream_t st)
 {
     typedef pgk::RowShape<NPHI> S;
-    dim3 grid(s->n_r / S::ROWS, batch);
-    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_tw_row, s->d_rs_out, s->n_r,
+    const int n_items = (s->n_r / S::ROWS) * batch;
+    const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
+    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_tw_row, s->d_rs_out, s->n_r, n_items,
                                                                  z_stride, phi_stride);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
@@ -204,6 +207,12 @@ pg_status prepare_rows(pg_solver *s)
                                     (int)S::SMEM));
     PG_CUDA(s, cudaFuncSetAttribute(pgk::rows_inv_kernel<NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)S::SMEM));
+    // persistent grid: as many CTAs as are resident at once (the smaller of the two kernels' occupancies)
+    int occ_f = 0, occ_i = 0;
+    PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, pgk::rows_fwd_kernel<NPHI>, S::THREADS, S::SMEM));
+    PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, pgk::rows_inv_kernel<NPHI>, S::THREADS, S::SMEM));
+    const int occ = occ_f < occ_i ? occ_f : occ_i;
+    s->row_ctas = (occ > 0 ? occ : 1) * s->sm_count;
     return PG_OK;
 }
 template <int NR>
@@ -422,6 +431,7 @@ pg_status create_impl(pg_solver *s)
     PG_CUDA(s, cudaSetDevice(s->device));
     cudaDeviceProp prop;
     PG_CUDA(s, cudaGetDeviceProperties(&prop, s->device));
+    s->sm_count = prop.multiProcessorCount;
     if (prop.major != 10) {
         set_err(s, "device %d is sm_%d%d; this library is built for sm_100a (B200) only and has no fallback",
                 s->device, prop.major, prop.minor);
