@@ -32,6 +32,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_2409_02294_b200.workloads import CONFIGS, make_sigma  # noqa: E402
+from paper_2409_02294_b200 import replicas  # noqa: E402
 
 METRIC = "potential solves/sec (fp64 FFT-convolution, log-polar thin disk)"
 UNIT = "solves/s"
@@ -95,8 +96,7 @@ class ClockSampler:
         return out
 
 
-def dist_env():
-    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+dist_env = replicas.dist_env
 
 
 # ------------------------------------------------------------------ CPU oracle legs
@@ -203,17 +203,10 @@ def run_ours(args):
         pg.pg_potential(h, d_phi[p], c.batch, pg.PG_MEM_DEVICE)
 
     def barrier():
-        if world > 1:
-            import torch.distributed as dist
-            dist.barrier()
+        replicas.barrier(world)
 
     def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        import torch.distributed as dist
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return replicas.max_over_ranks(x, world, "cuda")
 
     for k in range(args.warmup):
         step(k)
