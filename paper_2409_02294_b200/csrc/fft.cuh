@@ -268,17 +268,21 @@ struct Bases {
 };
 
 // ------------------------------------------------------------------ forward passes
-// fwd_a: v[jj] = x[u + T jj]  ->  pass A, results stored to the line (nothing stored, and v left
-// holding the rotated inputs, for one-pass plans).  No barrier.
+// Every pass comes in three parts -- load (shared memory -> v), compute (v in place, registers only),
+// store (v -> shared memory) -- so that a kernel can put its own synchronisation between them
+// (cols_kernel alternates the compute parts of two transforms, kernels.cuh).  The fused forms
+// fwd_a / fwd_b / ... below keep the older call sites short.
+//
+// pass A: v[jj] = x[u + T jj] on entry.  DFT g of the thread works on v[a GA + g], a < RA, in place:
+// output d of DFT g is left in v[d GA + g].  One-pass plans only rotate the inputs (ODD).
 template <int L, int KIND, bool ODD>
-__device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+__device__ __forceinline__ void fwd_a_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
-    constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
+    constexpr int RA = P::RA, GA = P::GA;
     if constexpr (P::NPASS == 1) {
         if constexpr (ODD) rotate_half<16, false>(v);
     } else {
-        cplx *base = line + pad<RC>(u);
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
@@ -289,47 +293,117 @@ __device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, co
             dft<RA, false>(x);
             apply_powers<RA, false, ODD>(x, s);
 #pragma unroll
+            for (int d = 0; d < RA; ++d) v[d * GA + g] = x[d];
+        }
+    }
+}
+template <int L, int KIND>
+__device__ __forceinline__ void fwd_a_store(const cplx (&v)[16], cplx *__restrict__ line, const int u)
+{
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
+    if constexpr (P::NPASS > 1) {
+        cplx *base = line + pad<RC>(u);
+#pragma unroll
+        for (int g = 0; g < GA; ++g) {
+#pragma unroll
             for (int d = 0; d < RA; ++d) {
-                if ((T * g) % RC == 0) base[pad<RC>(d * MA + T * g)] = x[d];
-                else line[pad<RC>(d * MA + u + T * g)] = x[d];
+                if ((T * g) % RC == 0) base[pad<RC>(d * MA + T * g)] = v[d * GA + g];
+                else line[pad<RC>(d * MA + u + T * g)] = v[d * GA + g];
             }
         }
     }
 }
+template <int L, int KIND, bool ODD>
+__device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+{
+    fwd_a_compute<L, KIND, ODD>(v, tw, u);
+    fwd_a_store<L, KIND>(v, line, u);
+}
 
-// fwd_b: pass B in place (three-pass plans; no-op otherwise).  Call after a barrier; no barrier inside.
+// pass B in place (three-pass plans; no-op otherwise): DFT h of the thread sits in v[h RB + a]
 template <int L, int KIND>
-__device__ __forceinline__ void fwd_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+__device__ __forceinline__ cplx *pass_b_base(cplx *__restrict__ line, const int u)
+{
+    typedef Plan<L, KIND> P;
+    return line + pad<P::RC>((u / P::RC) * P::MA) + u % P::RC;
+}
+template <int L, int KIND>
+__device__ __forceinline__ void pass_b_load(cplx (&v)[16], const cplx *__restrict__ base)
 {
     typedef Plan<L, KIND> P;
     if constexpr (P::NPASS == 3) {
         constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
-        const int bp = u % RC, da0 = u / RC;
-        cplx *base = line + pad<RC>(da0 * MA) + bp;
+#pragma unroll
+        for (int h = 0; h < GB; ++h)
+#pragma unroll
+            for (int a = 0; a < RB; ++a) v[h * RB + a] = base[pad<RC>((T / RC) * h * MA + a * RC)];
+    }
+}
+template <int L, int KIND>
+__device__ __forceinline__ void pass_b_store(const cplx (&v)[16], cplx *__restrict__ base)
+{
+    typedef Plan<L, KIND> P;
+    if constexpr (P::NPASS == 3) {
+        constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
+#pragma unroll
+        for (int h = 0; h < GB; ++h)
+#pragma unroll
+            for (int a = 0; a < RB; ++a) base[pad<RC>((T / RC) * h * MA + a * RC)] = v[h * RB + a];
+    }
+}
+template <int L, int KIND>
+__device__ __forceinline__ void fwd_b_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
+{
+    typedef Plan<L, KIND> P;
+    if constexpr (P::NPASS == 3) {
+        constexpr int RB = P::RB, GB = P::GB;
         const cplx s = tw.b(u);
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
-            cplx x[RB];
-#pragma unroll
-            for (int a = 0; a < RB; ++a) x[a] = base[pad<RC>((T / RC) * h * MA + a * RC)];
-            dft<RB, false>(x);
-            apply_powers<RB, false, false>(x, s);
-#pragma unroll
-            for (int d = 0; d < RB; ++d) base[pad<RC>((T / RC) * h * MA + d * RC)] = x[d];
+            dft<RB, false>(&v[h * RB]);
+            apply_powers<RB, false, false>(&v[h * RB], s);
         }
     }
 }
+// fwd_b: call after a barrier; no barrier inside
+template <int L, int KIND>
+__device__ __forceinline__ void fwd_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+{
+    if constexpr (Plan<L, KIND>::NPASS == 3) {
+        cplx v[16];
+        cplx *base = pass_b_base<L, KIND>(line, u);
+        pass_b_load<L, KIND>(v, base);
+        fwd_b_compute<L, KIND>(v, tw, u);
+        pass_b_store<L, KIND>(v, base);
+    }
+}
 
-// fwd_c (COL): after a barrier, thread u reads block u and runs the last radix-16:
-// v[c] = X[bin0(u) + T c].  One-pass plans transform the registers they are given.
+// pass C (COL): thread u owns block u = 16 consecutive slots
 template <int L>
-__device__ __forceinline__ void fwd_c_col(cplx (&v)[16], const cplx *__restrict__ line, const int u)
+__device__ __forceinline__ void pass_c_col_load(cplx (&v)[16], const cplx *__restrict__ line, const int u)
 {
     if constexpr (Plan<L, COL>::NPASS > 1) {
         const cplx *b = line + 17 * u;
 #pragma unroll
         for (int j = 0; j < 16; ++j) v[j] = b[j];
     }
+}
+template <int L>
+__device__ __forceinline__ void pass_c_col_store(const cplx (&v)[16], cplx *__restrict__ line, const int u)
+{
+    if constexpr (Plan<L, COL>::NPASS > 1) {
+        cplx *b = line + 17 * u;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) b[j] = v[j];
+    }
+}
+// fwd_c (COL): after a barrier, thread u reads block u and runs the last radix-16:
+// v[c] = X[bin0(u) + T c].  One-pass plans transform the registers they are given.
+template <int L>
+__device__ __forceinline__ void fwd_c_col(cplx (&v)[16], const cplx *__restrict__ line, const int u)
+{
+    pass_c_col_load<L>(v, line, u);
     dft<16, false>(v);
 }
 
@@ -350,11 +424,7 @@ template <int L>
 __device__ __forceinline__ void inv_c_col(cplx (&v)[16], cplx *__restrict__ line, const int u)
 {
     dft<16, true>(v);
-    if constexpr (Plan<L, COL>::NPASS > 1) {
-        cplx *b = line + 17 * u;
-#pragma unroll
-        for (int j = 0; j < 16; ++j) b[j] = v[j];
-    }
+    pass_c_col_store<L>(v, line, u);
 }
 
 template <int L>
@@ -368,46 +438,64 @@ __device__ __forceinline__ void inv_c_row(cplx (&v)[16], cplx *__restrict__ line
 }
 
 template <int L, int KIND>
-__device__ __forceinline__ void inv_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+__device__ __forceinline__ void inv_b_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     if constexpr (P::NPASS == 3) {
-        constexpr int RB = P::RB, GB = P::GB, T = P::T, MA = P::MA, RC = P::RC;
-        const int bp = u % RC, da0 = u / RC;
-        cplx *base = line + pad<RC>(da0 * MA) + bp;
+        constexpr int RB = P::RB, GB = P::GB;
         const cplx s = tw.b(u);
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
-            cplx x[RB];
-#pragma unroll
-            for (int d = 0; d < RB; ++d) x[d] = base[pad<RC>((T / RC) * h * MA + d * RC)];
-            apply_powers<RB, true, false>(x, s);
-            dft<RB, true>(x);
-#pragma unroll
-            for (int a = 0; a < RB; ++a) base[pad<RC>((T / RC) * h * MA + a * RC)] = x[a];
+            apply_powers<RB, true, false>(&v[h * RB], s);
+            dft<RB, true>(&v[h * RB]);
         }
     }
 }
+template <int L, int KIND>
+__device__ __forceinline__ void inv_b(cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+{
+    if constexpr (Plan<L, KIND>::NPASS == 3) {
+        cplx v[16];
+        cplx *base = pass_b_base<L, KIND>(line, u);
+        pass_b_load<L, KIND>(v, base);
+        inv_b_compute<L, KIND>(v, tw, u);
+        pass_b_store<L, KIND>(v, base);
+    }
+}
 
-// inv_a: after a barrier; v[jj] = sum_k X[k] exp(+2 pi i n k / L) (ODD: exp(+2 pi i n (2k+1) / 2L)), n = u + T jj
-template <int L, int KIND, bool ODD>
-__device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+// inverse pass A: load leaves input d of DFT g in v[d GA + g]; compute leaves element n = u + T jj in v[jj]:
+// v[jj] = sum_k X[k] exp(+2 pi i n k / L)  (ODD: exp(+2 pi i n (2k+1) / 2L))
+template <int L, int KIND>
+__device__ __forceinline__ void inv_a_load(cplx (&v)[16], const cplx *__restrict__ line, const int u)
 {
     typedef Plan<L, KIND> P;
     constexpr int RA = P::RA, GA = P::GA, T = P::T, MA = P::MA, RC = P::RC;
+    if constexpr (P::NPASS > 1) {
+        const cplx *base = line + pad<RC>(u);
+#pragma unroll
+        for (int g = 0; g < GA; ++g) {
+#pragma unroll
+            for (int d = 0; d < RA; ++d) {
+                if ((T * g) % RC == 0) v[d * GA + g] = base[pad<RC>(d * MA + T * g)];
+                else v[d * GA + g] = line[pad<RC>(d * MA + u + T * g)];
+            }
+        }
+    }
+}
+template <int L, int KIND, bool ODD>
+__device__ __forceinline__ void inv_a_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
+{
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA;
     if constexpr (P::NPASS == 1) {
         if constexpr (ODD) rotate_half<16, true>(v);
     } else {
-        const cplx *base = line + pad<RC>(u);
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
             const cplx s = tw.template a<ODD>(u, g);
 #pragma unroll
-            for (int d = 0; d < RA; ++d) {
-                if ((T * g) % RC == 0) x[d] = base[pad<RC>(d * MA + T * g)];
-                else x[d] = line[pad<RC>(d * MA + u + T * g)];
-            }
+            for (int d = 0; d < RA; ++d) x[d] = v[d * GA + g];
             apply_powers<RA, true, ODD>(x, s);
             dft<RA, true>(x);
             if constexpr (ODD) rotate_half<RA, true>(x);
@@ -415,6 +503,13 @@ __device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ li
             for (int a = 0; a < RA; ++a) v[a * GA + g] = x[a];
         }
     }
+}
+// inv_a: after a barrier
+template <int L, int KIND, bool ODD>
+__device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
+{
+    inv_a_load<L, KIND>(v, line, u);
+    inv_a_compute<L, KIND, ODD>(v, tw, u);
 }
 
 // slot of element n = u + T jj of the natural order (pass A's side of the line): thread u owns

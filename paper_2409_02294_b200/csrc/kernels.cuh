@@ -66,8 +66,8 @@ struct ColShape {
     static constexpr int STRIDE = P::LINE;
     static constexpr int THREADS = GROUPS * T;
     static constexpr size_t LINES = (size_t)GROUPS * STRIDE * sizeof(cplx);
-    static constexpr size_t KSTAGE = (size_t)GROUPS * L * sizeof(double);   // Khat slices of the CTA's modes
-    static constexpr size_t SMEM = LINES + KSTAGE + 16;                     // + one mbarrier
+    static constexpr size_t STAGE = (size_t)GROUPS * L * sizeof(double);    // Khat slices of the CTA's modes
+    static constexpr size_t SMEM = LINES + STAGE + 16;                      // + one mbarrier
     static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : (THREADS <= 128 ? 4 : 512 / THREADS);   // cap registers at 128/thread
 };
 
@@ -79,6 +79,16 @@ __device__ __forceinline__ void named_barrier(const int id, const int threads)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
+__device__ __forceinline__ void named_barrier_arrive(const int id, const int threads)
+{
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+// programmatic dependent launch: wait for the preceding kernel of the stream (no-op without the
+// launch attribute) / allow the following kernel's CTAs to be scheduled as this grid drains
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// orders this thread's view of earlier generic-proxy shared-memory accesses before an asynchronous copy
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // ---------------------------------------------------------------- bulk asynchronous copy (TMA, 1-D)
 // global -> shared, completion signalled on an mbarrier by transferred bytes
@@ -286,12 +296,20 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         cp_async_commit();
     };
 
+    // Sigma may come from the preceding kernel of the stream, and W is still read by it
+    pdl_wait();
+    pdl_launch_dependents();
     int item = blockIdx.x;
     if (item < n_items) prefetch(item);
+    auto row_scale = [&](const int it) {
+        return (rscale != nullptr && it < n_items) ? __ldg(&rscale[(it % items_per_field) * ROWS + rho]) : 1.0;
+    };
+    double sc_next = row_scale(item);
     for (; item < n_items; item += gridDim.x) {
         const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
         cplx v[16];
-        const double sc = (rscale != nullptr) ? __ldg(&rscale[i0 + rho]) : 1.0;
+        const double sc = sc_next;
+        sc_next = row_scale(item + gridDim.x);
         cp_async_wait_all();
 #pragma unroll
         for (int jj = 0; jj < 16; ++jj) v[jj] = stage[jj * S::THREADS];
@@ -359,6 +377,8 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
     };
     auto get = [&](const int slot) { return stage[slot * S::THREADS]; };
 
+    pdl_wait();                    // W is written by the preceding kernel of the stream
+    pdl_launch_dependents();
     int item = blockIdx.x;
     if (item < n_items) prefetch(item);
     for (; item < n_items; item += gridDim.x) {
@@ -420,7 +440,7 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     // the Khat slices of this CTA's modes are contiguous: one bulk asynchronous copy into shared
     // memory, issued now and waited for after the forward transform
     double *kstage = reinterpret_cast<double *>(smem_raw + S::LINES);
-    unsigned long long *kbar = reinterpret_cast<unsigned long long *>(smem_raw + S::LINES + S::KSTAGE);
+    unsigned long long *kbar = reinterpret_cast<unsigned long long *>(smem_raw + S::LINES + S::STAGE);
     if (tid == 0) mbar_init(kbar, 1);
     __syncthreads();
     if (tid == 0) {
@@ -429,6 +449,8 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
         bulk_load(kstage, Khat + (long)m0 * 2 * L, (unsigned)(nm * 2 * L * sizeof(double)), kbar);
     }
     const double *kh = kstage + g * L;
+    pdl_wait();
+    pdl_launch_dependents();
 
     cplx v[16];
 #pragma unroll

@@ -147,6 +147,25 @@ pg_status upload(pg_solver *s, T **dst, const std::vector<T> &src)
 }
 
 // ------------------------------------------------------------------ kernel dispatch
+// Launch with programmatic stream serialization: the kernel's CTAs may be scheduled while the
+// preceding kernel of the stream drains; every kernel calls griddepcontrol.wait before it touches
+// data that kernel may read or write (kernels.cuh, pdl_wait).
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <int NPHI>
 pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const double *rscale, int n_rows,
                           int batch, long sigma_stride, long z_stride, cudaStream_t st)
@@ -154,9 +173,8 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (n_rows / S::ROWS) * batch;      // persistent CTAs walk over the items
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
-    pgk::rows_fwd_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(sigma, Z, s->d_tw_row, rscale, n_rows, n_items,
-                                                                 sigma_stride, z_stride);
-    PG_CUDA(s, cudaGetLastError());
+    PG_CUDA(s, launch_pdl(pgk::rows_fwd_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, sigma, Z, s->d_tw_row,
+                          rscale, n_rows, n_items, sigma_stride, z_stride));
     s->launches++;
     return PG_OK;
 }
@@ -168,9 +186,8 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (s->n_r / S::ROWS) * batch;
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
-    pgk::rows_inv_kernel<NPHI><<<grid, S::THREADS, S::SMEM, st>>>(Z, phi, s->d_tw_row, s->d_rs_out, s->n_r, n_items,
-                                                                 z_stride, phi_stride);
-    PG_CUDA(s, cudaGetLastError());
+    PG_CUDA(s, launch_pdl(pgk::rows_inv_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, Z, phi, s->d_tw_row,
+                          s->d_rs_out, s->n_r, n_items, z_stride, phi_stride));
     s->launches++;
     return PG_OK;
 }
@@ -181,8 +198,8 @@ pg_status launch_cols(pg_solver *s, cplx *Z, int batch, long z_stride, cudaStrea
     typedef pgk::ColShape<NR> S;
     const int modes = s->half + 1;
     dim3 grid((modes + S::MODES - 1) / S::MODES, batch);
-    pgk::cols_kernel<NR><<<grid, S::THREADS, S::SMEM, st>>>(Z, s->d_khat, s->d_tw_col, modes, z_stride);
-    PG_CUDA(s, cudaGetLastError());
+    PG_CUDA(s, launch_pdl(pgk::cols_kernel<NR>, grid, dim3(S::THREADS), S::SMEM, st, Z, (const double *)s->d_khat,
+                          (const cplx *)s->d_tw_col, modes, z_stride));
     s->launches++;
     return PG_OK;
 }
