@@ -157,6 +157,22 @@ def run_reference(args):
     return 0
 
 
+def fp64_block(cfg, dom, ms_per_launch, clocks):
+    """Secondary roofline of the dominant kernel: FP64 thread instructions per second against the
+    pipe's issue peak 64 x SMs x SM clock (what actually bounds cols_kernel)."""
+    n = NCU_FP64_INSTR.get((cfg, dom))
+    if n is None or ms_per_launch <= 0:
+        return None
+    import torch
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    peak = FP64_LANES_PER_CLK_PER_SM * sms * mhz * 1e6
+    achieved = n / (ms_per_launch * 1e-3)
+    return {"bound": "alu", "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "T fp64 thread-instr/s",
+            "frac": achieved / peak, "thread_instructions_per_launch": n,
+            "peak_source": f"64 lanes/clk/SM x {sms} SMs x {mhz:.0f} MHz"}
+
+
 def workload_name(cfg: int) -> str:
     c = CONFIGS[cfg]
     return f"BASELINE.json configs[{cfg - 1}]: {c.name}, r in [{c.r_in:g},{c.r_out:g}], eps={c.eps:g}, batch {c.batch}"
@@ -316,6 +332,7 @@ def run_ours(args):
                         for i in range(pg.PG_NUM_KERNELS)},
             "path": {"alg_bytes_per_step": path_bytes, "gbs": path_gbs, "frac_of_peak": path_gbs / peak,
                      "frac_of_8TBs_nominal": path_gbs / 8000.0},
+            "fp64": fp64_block(cfg, dom, per_launch_ms[dom], clocks),
             "l2_flushed_ms_per_step": ms_flushed, "l2_flushed_frac_of_peak": path_bytes / (ms_flushed * 1e-3) / 1e9 / peak,
         },
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * c.batch,
@@ -342,7 +359,15 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), keyed by (config, kernel index).  Filled in from profiles/*.md; None = not captured.
-NCU_TRAFFIC: dict = {}
+NCU_TRAFFIC: dict = {          # profiles/r1_03_pdl.md
+    (5, 0): 33.6e6 + 1.4e6,    # rows_fwd_kernel<2048>
+    (5, 1): 67.2e6 + 0.9e6,    # cols_kernel<2048>
+    (5, 2): 33.6e6 + 0.6e6,    # rows_inv_kernel<2048>
+}
+# FP64 thread instructions (DADD + DMUL + DFMA) per launch from the same capture; the FP64 pipe issues
+# 64 per clock per SM (ncu sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained)
+NCU_FP64_INSTR: dict = {(5, 0): 0.97e8, (5, 1): 3.71e8, (5, 2): 0.97e8}
+FP64_LANES_PER_CLK_PER_SM = 64
 
 
 def main():
