@@ -155,6 +155,52 @@ __device__ __forceinline__ void dft(cplx *x)
     }
 }
 
+// ------------------------------------------------------------------ pruned radix-N DFTs (zero-padded transforms)
+// Forward DFT of N points whose upper half is zero: x[0..N/2) in, X[0..N) out (natural order).
+// The first decimation-in-frequency stage degenerates to a copy and a rotation.
+template <int N, int J = 0>
+__device__ __forceinline__ void zero_upper_stage(cplx *x)
+{
+    if constexpr (J < N / 2) {
+        x[J + N / 2] = mulroot<J * (32 / N), false>(x[J]);
+        zero_upper_stage<N, J + 1>(x);
+    }
+}
+template <int N>
+__device__ __forceinline__ void dft_zero_upper(cplx *x)
+{
+    static_assert(N >= 2 && N <= 32, "radix");
+    zero_upper_stage<N>(x);
+    Dif<N / 2, false>::run(x);
+    Dif<N / 2, false>::run(x + N / 2);
+    cplx y[N];
+#pragma unroll
+    for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
+#pragma unroll
+    for (int k = 0; k < N; ++k) x[k] = y[k];
+}
+// Inverse DFT of N points of which only the lower half of the outputs is wanted:
+// y[n] = sum_d X[d] exp(+2 pi i n d / N), n < N/2, left in x[0..N/2)  (decimation in time, last stage halved)
+template <int N, int K = 0>
+__device__ __forceinline__ void lower_half_stage(cplx *x, const cplx *e, const cplx *o)
+{
+    if constexpr (K < N / 2) {
+        x[K] = cadd(e[K], mulroot<K * (32 / N), true>(o[K]));
+        lower_half_stage<N, K + 1>(x, e, o);
+    }
+}
+template <int N>
+__device__ __forceinline__ void idft_lower_half(cplx *x)
+{
+    static_assert(N >= 2 && N <= 32, "radix");
+    cplx e[N / 2], o[N / 2];
+#pragma unroll
+    for (int d = 0; d < N / 2; ++d) { e[d] = x[2 * d]; o[d] = x[2 * d + 1]; }
+    dft<N / 2, true>(e);
+    dft<N / 2, true>(o);
+    lower_half_stage<N>(x, e, o);
+}
+
 // x[a] *= exp(-/+ i pi a / N), a < N  (the input rotation of the ODD transform; INV: the conjugate)
 template <int N, bool INV, int A = 1>
 __device__ __forceinline__ void rotate_half(cplx *x)
@@ -171,7 +217,7 @@ enum { COL = 0, ROW = 1 };
 template <int L, int KIND>
 struct Plan {
     static constexpr int RC = (KIND == ROW) ? 8 : 16;
-    static_assert(L >= 16 && L <= 2048 && (L & (L - 1)) == 0, "unsupported FFT length");
+    static_assert(L >= 16 && L <= 4096 && (L & (L - 1)) == 0, "unsupported FFT length");
     static constexpr int REST = L / RC;                                  // RA * RB
     static constexpr int NPASS = REST == 1 ? 1 : (REST <= 16 ? 2 : 3);
     static constexpr int RB = NPASS == 3 ? RC : 1;
@@ -319,6 +365,53 @@ __device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, co
 {
     fwd_a_compute<L, KIND, ODD>(v, tw, u);
     fwd_a_store<L, KIND>(v, line, u);
+}
+
+// Pass A of a transform whose input is zero in its upper half (the zero-padded radial transform):
+// only v[0..8) is read (element n = u + T jj < L/2); all 16 outputs are produced as in fwd_a_compute.
+template <int L, int KIND>
+__device__ __forceinline__ void fwd_a_compute_zero_upper(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
+{
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA;
+    static_assert(P::NPASS > 1 && RA >= 2, "zero-padded plans have at least two passes");
+    cplx y[16];
+#pragma unroll
+    for (int g = 0; g < GA; ++g) {
+        cplx x[RA];
+#pragma unroll
+        for (int a = 0; a < RA / 2; ++a) x[a] = v[a * GA + g];
+        const cplx s = tw.template a<false>(u, g);
+        dft_zero_upper<RA>(x);
+        apply_powers<RA, false, false>(x, s);
+#pragma unroll
+        for (int d = 0; d < RA; ++d) y[d * GA + g] = x[d];
+    }
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = y[j];
+}
+// Inverse pass A keeping only the lower half of the outputs (the crop back to L/2 points):
+// v[jj], jj < 8, is element n = u + T jj
+template <int L, int KIND>
+__device__ __forceinline__ void inv_a_compute_lower_half(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
+{
+    typedef Plan<L, KIND> P;
+    constexpr int RA = P::RA, GA = P::GA;
+    static_assert(P::NPASS > 1 && RA >= 2, "zero-padded plans have at least two passes");
+    cplx y[8];
+#pragma unroll
+    for (int g = 0; g < GA; ++g) {
+        cplx x[RA];
+        const cplx s = tw.template a<false>(u, g);
+#pragma unroll
+        for (int d = 0; d < RA; ++d) x[d] = v[d * GA + g];
+        apply_powers<RA, true, false>(x, s);
+        idft_lower_half<RA>(x);
+#pragma unroll
+        for (int a = 0; a < RA / 2; ++a) y[a * GA + g] = x[a];
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = y[j];
 }
 
 // pass B in place (three-pass plans; no-op otherwise): DFT h of the thread sits in v[h RB + a]

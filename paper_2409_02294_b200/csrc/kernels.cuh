@@ -9,9 +9,9 @@
 //                                         inside the last pass of the row kernel (fft.cuh, ROW plans).
 //                                         The column kernel transforms W in place; the inverse row kernel
 //                                         re-packs and transforms back.
-//   Khat       : [H+1][2][n_r] real       spectrum of the Green's kernel for azimuthal mode m, split into
-//                                         the even (2k) and odd (2k+1) bins of the 2 n_r-point padded
-//                                         radial transform, STORED IN THE ORDER THE COLUMN KERNEL HOLDS THEM
+//   Khat       : [H+1][2 n_r] real        spectrum of the Green's kernel for azimuthal mode m over the bins of
+//                                         the 2 n_r-point padded radial transform, STORED IN THE ORDER THE
+//                                         COLUMN KERNEL HOLDS THEM
 //                                         (entry c T + u is bin  bin0(u) + T c); all normalisations folded in
 //   tw_row, tw_col : compact twiddle tables (Plan<L,KIND>::TW_*), long double on the host
 #pragma once
@@ -34,8 +34,8 @@ __host__ __device__ constexpr int rows_per_cta(int nphi)
 // azimuthal modes per CTA in the r pass
 __host__ __device__ constexpr int modes_per_cta(int nr)
 {
-    const int T = nr / 16;
-    const int c = 128 / T;
+    const int T = nr / 8;          // threads of one 2 n_r-point transform
+    const int c = 256 / T;
     return c < 1 ? 1 : (c > 8 ? 8 : c);
 }
 // Shared-memory slots between the lines of two rows of a CTA.  In the row-fastest pass a
@@ -58,15 +58,14 @@ struct RowShape {
 };
 template <int NR>
 struct ColShape {
-    static constexpr int L = NR;
+    static constexpr int L = 2 * NR;                        // the zero-padded radial transform
     typedef Plan<L, COL> P;
-    static constexpr int T = P::T;
+    static constexpr int T = P::T;                          // threads per mode = n_r / 8
     static constexpr int MODES = modes_per_cta(NR);
-    static constexpr int GROUPS = 2 * MODES;                // (mode, branch)
     static constexpr int STRIDE = P::LINE;
-    static constexpr int THREADS = GROUPS * T;
-    static constexpr size_t LINES = (size_t)GROUPS * STRIDE * sizeof(cplx);
-    static constexpr size_t STAGE = (size_t)GROUPS * L * sizeof(double);    // Khat slices of the CTA's modes
+    static constexpr int THREADS = MODES * T;
+    static constexpr size_t LINES = (size_t)MODES * STRIDE * sizeof(cplx);
+    static constexpr size_t STAGE = (size_t)MODES * L * sizeof(double);     // Khat slices of the CTA's modes
     static constexpr size_t SMEM = LINES + STAGE + 16;                      // + one mbarrier
     static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : (THREADS <= 128 ? 4 : 512 / THREADS);   // cap registers at 128/thread
 };
@@ -409,33 +408,29 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
 // One CTA owns MODES azimuthal modes; mode m is the column x[0..n_r) = W[m][.].  It is convolved
 // with the Green's kernel over the radial lags, zero-padded to 2 n_r, and cropped back to n_r:
 //   y[n] = (1/2N) sum_{k'<2N} Khat[k'] Xpad[k'] e^{+2 pi i k' n / 2N},   n < N = n_r.
-// The padded 2N-point transform with a zero upper half and a cropped output is exactly two N-point
-// problems (decimation in frequency forward / in time backward), one per thread group ("branch"):
-//   even bins: FFT_N(x)   * Khat[2k]    -> IFFT_N    -> e[n]
-//   odd  bins: OFFT_N(x)  * Khat[2k+1]  -> IOFFT_N   -> o[n]      (odd-frequency transform, fft.cuh)
-//   y[n] = e[n] + o[n]                  (1/2N folded into Khat)
-// so the padded array and the discarded half are never formed (a3: multiply fused into the last
-// forward pass; a4: inverse with fused crop).  The two branches run on two thread groups with their
-// own named barriers; they meet once, at the end, where each group adds and stores half of y.
+// The 2N-point transform is carried by T = N/8 threads with 16 spectrum bins each, but a thread reads
+// only 8 column elements (the upper half of the padded input is zero: pass A starts from a pruned
+// radix-RA DFT, fft.cuh dft_zero_upper) and writes only 8 (the crop: the last inverse pass keeps the
+// lower half of its outputs, idft_lower_half).  The padded array and the discarded half are never
+// formed in memory (a3: multiply fused into the last forward pass; a4: inverse with fused crop).
 template <int NR>
 __global__ void __launch_bounds__(ColShape<NR>::THREADS, ColShape<NR>::MIN_CTAS)
 cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw, const int n_modes,
             const long w_field_stride)
 {
     typedef ColShape<NR> S;
-    typedef Plan<NR, COL> P;
+    typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
 
     const int tid = threadIdx.x;
-    const int u = tid % T, g = tid / T;
-    const int br = g & 1, ml = g >> 1;
+    const int u = tid % T, ml = tid / T;
     const int m_raw = blockIdx.x * S::MODES + ml;
     const bool live = m_raw < n_modes;
     const int mode = live ? m_raw : n_modes - 1;
-    cplx *line = smem + g * S::STRIDE;
-    cplx *col = W + blockIdx.y * w_field_stride + (long)mode * L;
+    cplx *line = smem + ml * S::STRIDE;
+    cplx *col = W + blockIdx.y * w_field_stride + (long)mode * NR;
 
     // the Khat slices of this CTA's modes are contiguous: one bulk asynchronous copy into shared
     // memory, issued now and waited for after the forward transform
@@ -446,26 +441,26 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     if (tid == 0) {
         const int m0 = blockIdx.x * S::MODES;
         const int nm = (n_modes - m0 < S::MODES) ? n_modes - m0 : S::MODES;
-        bulk_load(kstage, Khat + (long)m0 * 2 * L, (unsigned)(nm * 2 * L * sizeof(double)), kbar);
+        bulk_load(kstage, Khat + (long)m0 * L, (unsigned)(nm * L * sizeof(double)), kbar);
     }
-    const double *kh = kstage + g * L;
-    pdl_wait();
+    const double *kh = kstage + ml * L;
+    pdl_wait();                    // W is written by the preceding kernel of the stream
     pdl_launch_dependents();
 
     cplx v[16];
 #pragma unroll
-    for (int jj = 0; jj < 16; ++jj) v[jj] = col[u + T * jj];
+    for (int jj = 0; jj < 8; ++jj) v[jj] = col[u + T * jj];
     Bases<L, COL> bases;
-    bases.load(tw, u, br != 0);
+    bases.load(tw, u, false);
 
-    const Sync<T, S::THREADS> sync(g + 1);
-    if (br) fwd_a<L, COL, true>(v, line, bases, u);
-    else fwd_a<L, COL, false>(v, line, bases, u);
+    const Sync<T, S::THREADS> sync(ml + 1);
+    fwd_a_compute_zero_upper<L, COL>(v, bases, u);
+    fwd_a_store<L, COL>(v, line, u);
     if constexpr (P::NPASS == 3) {
         sync();
         fwd_b<L, COL>(line, bases, u);
     }
-    if constexpr (P::NPASS > 1) sync();
+    sync();
     fwd_c_col<L>(v, line, u);
     mbar_wait(kbar, 0);
 #pragma unroll
@@ -476,26 +471,16 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     }
     // inv_c writes exactly the 16 slots this thread has just read: no barrier in between
     inv_c_col<L>(v, line, u);
-    if constexpr (P::NPASS > 1) sync();
+    sync();
     if constexpr (P::NPASS == 3) {
         inv_b<L, COL>(line, bases, u);
         sync();
     }
-    if (br) inv_a<L, COL, true>(v, line, bases, u);
-    else inv_a<L, COL, false>(v, line, bases, u);
-
-    // y = e + o: group `br` finishes elements jj in [8 br, 8 br + 8) and hands the other eight to its
-    // partner through the slots it owns (nobody else touches them after pass A)
-#pragma unroll
-    for (int jj = 0; jj < 16; ++jj)
-        if ((jj >> 3) != br) line[own_slot<L, COL>(u, jj)] = v[jj];
-    if constexpr (T >= 32 && 2 * T < S::THREADS) named_barrier(9 + ml, 2 * T);
-    else __syncthreads();
-    const cplx *other = smem + (g ^ 1) * S::STRIDE;
+    inv_a_load<L, COL>(v, line, u);
+    inv_a_compute_lower_half<L, COL>(v, bases, u);
     if (live) {
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj)
-            if ((jj >> 3) == br) col[u + T * jj] = cadd(v[jj], other[own_slot<L, COL>(u, jj)]);
+        for (int jj = 0; jj < 8; ++jj) col[u + T * jj] = v[jj];
     }
 }
 
@@ -520,45 +505,37 @@ __global__ void green_fill_kernel(double *__restrict__ Kpad, const int n_r, cons
 }
 
 // Column pass of the kernel spectrum (one-time, a1).  WK[m][0..2N) is azimuthal mode m of the padded
-// kernel Kpad (2N rows, from rows_fwd_kernel).  Its 2N-point forward transform is taken as the even
-// bins FFT_N(x[n] + x[n+N]) and the odd bins OFFT_N(x[n] - x[n+N]), exactly as cols_kernel consumes
-// them and in the order it holds them; the real part is scaled and stored:
-//   Khat[m][br][c T + u] = scale Re X[2 (bin0(u) + T c) + br].
+// kernel Kpad (2N rows, from rows_fwd_kernel).  Its 2N-point forward transform is taken with the plan
+// cols_kernel uses (no pruning here: all 2N lags are populated), and the real part is scaled and stored
+// in the order cols_kernel holds the bins:   Khat[m][c T + u] = scale Re X[bin0(u) + T c].
 // (K is even in both lags, so X is real up to rounding.)
 template <int NR>
-__global__ void __launch_bounds__(2 * (NR / 16))
+__global__ void __launch_bounds__(NR / 8)
 khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const cplx *__restrict__ tw, const double scale)
 {
-    typedef Plan<NR, COL> P;
-    constexpr int L = NR, T = L / 16, STRIDE = P::LINE;
+    constexpr int L = 2 * NR;
+    typedef Plan<L, COL> P;
+    constexpr int T = P::T;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx *smem = reinterpret_cast<cplx *>(smem_raw);
+    cplx *line = reinterpret_cast<cplx *>(smem_raw);
 
-    const int tid = threadIdx.x;
-    const int u = tid % T, br = tid / T;
+    const int u = threadIdx.x;
     const int m = blockIdx.x;                         // mode 0..H
-    const cplx *col = WK + (long)m * (2 * L);
-    cplx *line = smem + br * STRIDE;
+    const cplx *col = WK + (long)m * L;
 
     cplx v[16];
 #pragma unroll
-    for (int jj = 0; jj < 16; ++jj) {
-        const int n = u + T * jj;
-        const cplx x1 = col[n], x2 = col[n + L];
-        v[jj] = br ? csub(x1, x2) : cadd(x1, x2);
-    }
+    for (int jj = 0; jj < 16; ++jj) v[jj] = col[u + T * jj];
     Bases<L, COL> bases;
-    bases.load(tw, u, br != 0);
-    const Sync<T, 2 * T> sync(br + 1);
-    if (br) fwd_a<L, COL, true>(v, line, bases, u);
-    else fwd_a<L, COL, false>(v, line, bases, u);
+    bases.load(tw, u, false);
+    fwd_a<L, COL, false>(v, line, bases, u);
     if constexpr (P::NPASS == 3) {
-        sync();
+        __syncthreads();
         fwd_b<L, COL>(line, bases, u);
     }
-    if constexpr (P::NPASS > 1) sync();
+    __syncthreads();
     fwd_c_col<L>(v, line, u);
-    double *kh = Khat + ((long)m * 2 + br) * L;
+    double *kh = Khat + (long)m * L;
 #pragma unroll
     for (int k = 0; k < 16; ++k) kh[u + T * k] = scale * v[k].x;
 }

@@ -44,7 +44,7 @@ struct pg_solver {
     cplx *d_W = nullptr;          // W: [max_batch][half+1][n_r]
     double *d_khat = nullptr;     // [half+1][2][n_r]
     cplx *d_tw_row = nullptr;     // Plan<n_phi/2, ROW> twiddle table
-    cplx *d_tw_col = nullptr;     // Plan<n_r, COL> twiddle table
+    cplx *d_tw_col = nullptr;     // Plan<2 n_r, COL> twiddle table
     double *d_rs_in = nullptr, *d_rs_out = nullptr;
     double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
     double *d_sigma_own = nullptr, *d_phi_own = nullptr;   // [max_batch][n_r][n_phi], lazily allocated
@@ -134,6 +134,7 @@ bool twiddles_for(int len, std::vector<cplx> &tw)
         case 512: fill_twiddles<512, KIND>(tw); return true;
         case 1024: fill_twiddles<1024, KIND>(tw); return true;
         case 2048: fill_twiddles<2048, KIND>(tw); return true;
+        case 4096: if (KIND == pgk::COL) { fill_twiddles<4096, pgk::COL>(tw); return true; } return false;
         default: return false;
     }
 }
@@ -207,8 +208,8 @@ pg_status launch_cols(pg_solver *s, cplx *Z, int batch, long z_stride, cudaStrea
 template <int NR>
 pg_status launch_khat_cols(pg_solver *s, const cplx *ZK, double scale, cudaStream_t st)
 {
-    const int threads = 2 * (NR / 16);
-    const size_t smem = 2 * (size_t)pgk::Plan<NR, pgk::COL>::LINE * sizeof(cplx);
+    const int threads = NR / 8;
+    const size_t smem = (size_t)pgk::Plan<2 * NR, pgk::COL>::LINE * sizeof(cplx);
     pgk::khat_cols_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, s->d_khat, s->d_tw_col, scale);
     PG_CUDA(s, cudaGetLastError());
     s->launches++;
@@ -239,7 +240,7 @@ pg_status prepare_cols(pg_solver *s)
     PG_CUDA(s, cudaFuncSetAttribute(pgk::cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)S::SMEM));
     PG_CUDA(s, cudaFuncSetAttribute(pgk::khat_cols_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)(2 * pgk::Plan<NR, pgk::COL>::LINE * sizeof(cplx))));
+                                    (int)(pgk::Plan<2 * NR, pgk::COL>::LINE * sizeof(cplx))));
     return PG_OK;
 }
 
@@ -482,7 +483,7 @@ pg_status create_impl(pg_solver *s)
     // FFT tables: base roots of the packed row transform (length n_phi/2) and of the n_r-point
     // column transforms (even and odd-frequency variants), in the layout Plan<L,KIND>::TW_* expects
     std::vector<cplx> tw_row, tw_col;
-    if (!twiddles_for<pgk::ROW>(s->half, tw_row) || !twiddles_for<pgk::COL>(n_r, tw_col)) {
+    if (!twiddles_for<pgk::ROW>(s->half, tw_row) || !twiddles_for<pgk::COL>(2 * n_r, tw_col)) {
         set_err(s, "unsupported transform length");
         return PG_ERR_UNSUPPORTED;
     }
