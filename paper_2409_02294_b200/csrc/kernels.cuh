@@ -20,6 +20,9 @@
 #ifndef PG_ROW_THREADS
 #define PG_ROW_THREADS 128
 #endif
+#ifndef PG_ROW_THREADS_BIG
+#define PG_ROW_THREADS_BIG 256      // n_phi >= 2048: 4 rows per CTA (64-byte runs in W), one CTA per SM
+#endif
 
 namespace pgk {
 
@@ -28,7 +31,7 @@ namespace pgk {
 __host__ __device__ constexpr int rows_per_cta(int nphi)
 {
     const int T = nphi / 32;
-    const int r = PG_ROW_THREADS / (T > 0 ? T : 1);
+    const int r = (nphi >= 2048 ? PG_ROW_THREADS_BIG : PG_ROW_THREADS) / (T > 0 ? T : 1);
     return r < 2 ? 2 : (r > 16 ? 16 : r);
 }
 // azimuthal modes per CTA in the r pass
