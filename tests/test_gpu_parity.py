@@ -214,3 +214,49 @@ def test_zero_density_gives_zero_potential():
         assert np.all(d.solve(np.zeros((64, 64))) == 0.0)
     finally:
         d.close()
+
+
+# ---------------------------------------------------------------- the launch configuration bench.py times
+@pytest.mark.parametrize("cfg", [3, 5])
+def test_back_to_back_solves_equal_isolated_solves(cfg):
+    """bench.py enqueues solves back to back on one stream, rotating over distinct (Sigma, Phi) buffers,
+    with the kernels chained by programmatic dependent launch (rows_fwd of solve n+1 is scheduled
+    while rows_inv of solve n drains, and both use the one W workspace).  Every result of the chain
+    must equal, bit for bit, the result of the same solve run alone, and sampled rings must meet the
+    oracle at north_star's tolerance."""
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, _ = d.s.grid()
+        base = make_sigma(cfg, r, phi)
+        fields = [np.ascontiguousarray(np.roll(base, 37 * k, axis=1) * (1.0 + 0.1 * k)) for k in range(6)]
+        alone = [d.solve(f) for f in fields]
+        d_s = [torch.from_numpy(f).cuda() for f in fields]
+        d_p = [torch.empty_like(t) for t in d_s]
+        torch.cuda.synchronize()
+        for rep in range(3):                      # 18 solves enqueued without any synchronisation
+            for k in range(6):
+                pg.pg_set_density(d.s.h, d_s[k], 1, pg.PG_MEM_DEVICE)
+                pg.pg_potential(d.s.h, d_p[k], 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(d.s.h)
+        for k in range(6):
+            assert np.array_equal(d_p[k].cpu().numpy(), alone[k]), f"chained solve {k} differs from the isolated one"
+        rings = np.array([0, 1, c.n_r // 2, c.n_r - 1], dtype=np.int32)
+        ref = oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, fields[3], rings)
+        assert_parity(alone[3][rings], ref, f"config {cfg} chained, sampled rings")
+    finally:
+        d.close()
+
+
+def test_partial_batch_uses_the_first_fields_only():
+    """A solver created for max_batch = 4 solves batches of 1..4; field b of any batch equals the single solve."""
+    d = Dev(128, 256, 1.0, 50.0, 0.01, max_batch=4)
+    try:
+        fields = np.stack([random_sigma(128, 256, seed=90 + b) for b in range(4)])
+        single = [d.solve(fields[b]) for b in range(4)]
+        for nb in (1, 2, 3, 4):
+            got = d.solve(fields[:nb])
+            got = got.reshape(nb, 128, 256)
+            for b in range(nb):
+                assert np.array_equal(got[b], single[b]), f"batch of {nb}, field {b}"
+    finally:
+        d.close()
