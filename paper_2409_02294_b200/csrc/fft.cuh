@@ -24,11 +24,10 @@
 //        holds bin k together with bin L - k, which is what the real-data split ("untangle") of a
 //        packed real transform needs, so that split costs no extra exchange.
 //
-// ODD variant of pass A (COL plans): computes the odd-frequency transform
-//        X[k] = sum_n x[n] exp(-2 pi i n (2k+1) / 2L)
-// i.e. the odd bins of the 2L-point transform of x zero-padded to 2L, by rotating the inputs of each
-// radix-RA DFT by exp(-i pi a / RA) (compile-time constants) and using odd powers of the inter-pass
-// twiddle.  No modulation table, no extra multiplies.
+// Zero-padded transforms (COL plans): the input's upper half is zero and only the lower half of the
+// inverse is wanted, so pass A starts from a pruned radix-RA DFT (dft_zero_upper) and the last inverse
+// pass ends in one (idft_lower_half): a thread then moves 8 elements to and from global memory while
+// it holds 16 spectrum bins in between.
 //
 // Twiddles: a thread loads only BASE roots (one per DFT of pass A, one for pass B) from small
 // compact tables built on the host in long double, and forms the powers it needs by two interleaved
@@ -201,16 +200,6 @@ __device__ __forceinline__ void idft_lower_half(cplx *x)
     lower_half_stage<N>(x, e, o);
 }
 
-// x[a] *= exp(-/+ i pi a / N), a < N  (the input rotation of the ODD transform; INV: the conjugate)
-template <int N, bool INV, int A = 1>
-__device__ __forceinline__ void rotate_half(cplx *x)
-{
-    if constexpr (A < N) {
-        x[A] = mulroot<A * (16 / N), INV>(x[A]);
-        rotate_half<N, INV, A + 1>(x);
-    }
-}
-
 // ------------------------------------------------------------------ plan
 enum { COL = 0, ROW = 1 };
 
@@ -231,8 +220,7 @@ struct Plan {
     static constexpr int LINE = L + L / RC;          // padded slots per transform
     // compact twiddle table of a transform (host: polargrav.cu fills it in this order)
     static constexpr int TW_A = 0;                   // [MA]  exp(-2 pi i b / L)
-    static constexpr int TW_AODD = MA;               // [MA]  exp(-2 pi i b / 2L)          (COL only)
-    static constexpr int TW_B = (KIND == COL) ? 2 * MA : MA;   // [RC]  exp(-2 pi i b' / MA)
+    static constexpr int TW_B = MA;                  // [RC]  exp(-2 pi i b' / MA)
     static constexpr int TW_UN = TW_B + RC;          // [NB]  i exp(-2 pi i q / 2L)         (ROW only)
     static constexpr int TW_LEN = TW_UN + ((KIND == ROW) ? NB : 0);
     static_assert(NPASS < 3 || T % RC == 0, "pass B mapping needs T to be a multiple of RC");
@@ -261,38 +249,26 @@ struct Sync {
 };
 
 // ------------------------------------------------------------------ twiddle powers
-// EVEN: x[d] *= s^d      (CONJ: conj(s)^d),       d = 0..K-1
-// ODD : x[d] *= s^(2d+1) (CONJ: conj),            d = 0..K-1
-// Two interleaved chains advanced by the same step keep the dependency depth at K/2.
-template <int K, bool CONJ, bool ODD>
+// x[d] *= s^d  (CONJ: conj(s)^d),  d = 0..K-1.  Two interleaved chains advanced by the same step
+// (s^2) keep the dependency depth at K/2.
+template <int K, bool CONJ>
 __device__ __forceinline__ void apply_powers(cplx *x, const cplx s)
 {
     if constexpr (K >= 2) {
         const cplx s2 = csq(s);
-        cplx a, b, step;
-        if constexpr (ODD) {
-            a = s;                 // s^1, s^5, ...   (even d)
-            b = cmul(s, s2);       // s^3, s^7, ...   (odd d)
-            step = csq(s2);        // s^4
-            x[0] = CONJ ? cmulc(x[0], a) : cmul(x[0], a);
-        } else {
-            a = s2;                // s^2, s^4, ...   (even d >= 2)
-            b = s;                 // s^1, s^3, ...   (odd d)
-            step = s2;
-        }
+        cplx a = s2;               // s^2, s^4, ...   (even d >= 2)
+        cplx b = s;                // s^1, s^3, ...   (odd d)
         x[1] = CONJ ? cmulc(x[1], b) : cmul(x[1], b);
 #pragma unroll
         for (int d = 2; d < K; ++d) {
             if (d & 1) {
-                b = cmul(b, step);
+                b = cmul(b, s2);
                 x[d] = CONJ ? cmulc(x[d], b) : cmul(x[d], b);
             } else {
-                if (ODD || d > 2) a = cmul(a, step);
+                if (d > 2) a = cmul(a, s2);
                 x[d] = CONJ ? cmulc(x[d], a) : cmul(x[d], a);
             }
         }
-    } else if constexpr (ODD) {
-        x[0] = CONJ ? cmulc(x[0], s) : cmul(x[0], s);
     }
 }
 
@@ -305,11 +281,7 @@ struct Bases {
     typedef Plan<L, KIND> P;
     const cplx *tw;
     __device__ __forceinline__ void load(const cplx *__restrict__ table, const int, const bool) { tw = table; }
-    template <bool ODD>
-    __device__ __forceinline__ cplx a(const int u, const int g) const
-    {
-        return __ldg(tw + (ODD ? P::TW_AODD : P::TW_A) + u + P::T * g);
-    }
+    __device__ __forceinline__ cplx a(const int u, const int g) const { return __ldg(tw + P::TW_A + u + P::T * g); }
     __device__ __forceinline__ cplx b(const int u) const { return __ldg(tw + P::TW_B + u % P::RC); }
 };
 
@@ -320,24 +292,21 @@ struct Bases {
 // fwd_a / fwd_b / ... below keep the older call sites short.
 //
 // pass A: v[jj] = x[u + T jj] on entry.  DFT g of the thread works on v[a GA + g], a < RA, in place:
-// output d of DFT g is left in v[d GA + g].  One-pass plans only rotate the inputs (ODD).
-template <int L, int KIND, bool ODD>
+// output d of DFT g is left in v[d GA + g].  One-pass plans do nothing here.
+template <int L, int KIND>
 __device__ __forceinline__ void fwd_a_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     constexpr int RA = P::RA, GA = P::GA;
-    if constexpr (P::NPASS == 1) {
-        if constexpr (ODD) rotate_half<16, false>(v);
-    } else {
+    if constexpr (P::NPASS > 1) {
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
 #pragma unroll
             for (int a = 0; a < RA; ++a) x[a] = v[a * GA + g];
-            const cplx s = tw.template a<ODD>(u, g);
-            if constexpr (ODD) rotate_half<RA, false>(x);
+            const cplx s = tw.a(u, g);
             dft<RA, false>(x);
-            apply_powers<RA, false, ODD>(x, s);
+            apply_powers<RA, false>(x, s);
 #pragma unroll
             for (int d = 0; d < RA; ++d) v[d * GA + g] = x[d];
         }
@@ -360,10 +329,10 @@ __device__ __forceinline__ void fwd_a_store(const cplx (&v)[16], cplx *__restric
         }
     }
 }
-template <int L, int KIND, bool ODD>
+template <int L, int KIND>
 __device__ __forceinline__ void fwd_a(cplx (&v)[16], cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
-    fwd_a_compute<L, KIND, ODD>(v, tw, u);
+    fwd_a_compute<L, KIND>(v, tw, u);
     fwd_a_store<L, KIND>(v, line, u);
 }
 
@@ -381,9 +350,9 @@ __device__ __forceinline__ void fwd_a_compute_zero_upper(cplx (&v)[16], const Ba
         cplx x[RA];
 #pragma unroll
         for (int a = 0; a < RA / 2; ++a) x[a] = v[a * GA + g];
-        const cplx s = tw.template a<false>(u, g);
+        const cplx s = tw.a(u, g);
         dft_zero_upper<RA>(x);
-        apply_powers<RA, false, false>(x, s);
+        apply_powers<RA, false>(x, s);
 #pragma unroll
         for (int d = 0; d < RA; ++d) y[d * GA + g] = x[d];
     }
@@ -402,10 +371,10 @@ __device__ __forceinline__ void inv_a_compute_lower_half(cplx (&v)[16], const Ba
 #pragma unroll
     for (int g = 0; g < GA; ++g) {
         cplx x[RA];
-        const cplx s = tw.template a<false>(u, g);
+        const cplx s = tw.a(u, g);
 #pragma unroll
         for (int d = 0; d < RA; ++d) x[d] = v[d * GA + g];
-        apply_powers<RA, true, false>(x, s);
+        apply_powers<RA, true>(x, s);
         idft_lower_half<RA>(x);
 #pragma unroll
         for (int a = 0; a < RA / 2; ++a) y[a * GA + g] = x[a];
@@ -455,7 +424,7 @@ __device__ __forceinline__ void fwd_b_compute(cplx (&v)[16], const Bases<L, KIND
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
             dft<RB, false>(&v[h * RB]);
-            apply_powers<RB, false, false>(&v[h * RB], s);
+            apply_powers<RB, false>(&v[h * RB], s);
         }
     }
 }
@@ -539,7 +508,7 @@ __device__ __forceinline__ void inv_b_compute(cplx (&v)[16], const Bases<L, KIND
         const cplx s = tw.b(u);
 #pragma unroll
         for (int h = 0; h < GB; ++h) {
-            apply_powers<RB, true, false>(&v[h * RB], s);
+            apply_powers<RB, true>(&v[h * RB], s);
             dft<RB, true>(&v[h * RB]);
         }
     }
@@ -557,7 +526,7 @@ __device__ __forceinline__ void inv_b(cplx *__restrict__ line, const Bases<L, KI
 }
 
 // inverse pass A: load leaves input d of DFT g in v[d GA + g]; compute leaves element n = u + T jj in v[jj]:
-// v[jj] = sum_k X[k] exp(+2 pi i n k / L)  (ODD: exp(+2 pi i n (2k+1) / 2L))
+// v[jj] = sum_k X[k] exp(+2 pi i n k / L)
 template <int L, int KIND>
 __device__ __forceinline__ void inv_a_load(cplx (&v)[16], const cplx *__restrict__ line, const int u)
 {
@@ -575,34 +544,31 @@ __device__ __forceinline__ void inv_a_load(cplx (&v)[16], const cplx *__restrict
         }
     }
 }
-template <int L, int KIND, bool ODD>
+template <int L, int KIND>
 __device__ __forceinline__ void inv_a_compute(cplx (&v)[16], const Bases<L, KIND> &tw, const int u)
 {
     typedef Plan<L, KIND> P;
     constexpr int RA = P::RA, GA = P::GA;
-    if constexpr (P::NPASS == 1) {
-        if constexpr (ODD) rotate_half<16, true>(v);
-    } else {
+    if constexpr (P::NPASS > 1) {
 #pragma unroll
         for (int g = 0; g < GA; ++g) {
             cplx x[RA];
-            const cplx s = tw.template a<ODD>(u, g);
+            const cplx s = tw.a(u, g);
 #pragma unroll
             for (int d = 0; d < RA; ++d) x[d] = v[d * GA + g];
-            apply_powers<RA, true, ODD>(x, s);
+            apply_powers<RA, true>(x, s);
             dft<RA, true>(x);
-            if constexpr (ODD) rotate_half<RA, true>(x);
 #pragma unroll
             for (int a = 0; a < RA; ++a) v[a * GA + g] = x[a];
         }
     }
 }
 // inv_a: after a barrier
-template <int L, int KIND, bool ODD>
+template <int L, int KIND>
 __device__ __forceinline__ void inv_a(cplx (&v)[16], const cplx *__restrict__ line, const Bases<L, KIND> &tw, const int u)
 {
     inv_a_load<L, KIND>(v, line, u);
-    inv_a_compute<L, KIND, ODD>(v, tw, u);
+    inv_a_compute<L, KIND>(v, tw, u);
 }
 
 // slot of element n = u + T jj of the natural order (pass A's side of the line): thread u owns

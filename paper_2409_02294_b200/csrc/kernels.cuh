@@ -320,7 +320,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) { v[jj].x *= sc; v[jj].y *= sc; }
         }
-        fwd_a<L, ROW, false>(v, line, bases, u);
+        fwd_a<L, ROW>(v, line, bases, u);
         if constexpr (P::NPASS == 3) {
             const Sync<T, S::THREADS> sync(rho + 1);
             sync();
@@ -399,7 +399,7 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
             inv_b<L, ROW>(line, bases, u);
             sync();
         }
-        inv_a<L, ROW, false>(v, line, bases, u);
+        inv_a<L, ROW>(v, line, bases, u);
         cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * NPHI);
 #pragma unroll
         for (int jj = 0; jj < 16; ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
@@ -531,7 +531,7 @@ khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const c
     for (int jj = 0; jj < 16; ++jj) v[jj] = col[u + T * jj];
     Bases<L, COL> bases;
     bases.load(tw, u, false);
-    fwd_a<L, COL, false>(v, line, bases, u);
+    fwd_a<L, COL>(v, line, bases, u);
     if constexpr (P::NPASS == 3) {
         __syncthreads();
         fwd_b<L, COL>(line, bases, u);

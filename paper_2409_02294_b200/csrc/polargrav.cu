@@ -111,7 +111,6 @@ void fill_twiddles(std::vector<cplx> &tw)
     tw.assign(P::TW_LEN, make_double2(0.0, 0.0));
     for (int b = 0; b < P::MA; ++b) {
         tw[P::TW_A + b] = unit((long double)b / L);
-        if (KIND == pgk::COL) tw[P::TW_AODD + b] = unit((long double)b / (2.0L * L));
     }
     for (int b = 0; b < P::RC; ++b) tw[P::TW_B + b] = unit((long double)b / P::MA);
     if (KIND == pgk::ROW) {
