@@ -260,3 +260,25 @@ def test_partial_batch_uses_the_first_fields_only():
                 assert np.array_equal(got[b], single[b]), f"batch of {nb}, field {b}"
     finally:
         d.close()
+
+
+@pytest.mark.parametrize("n_r,n_phi,batch", [(64, 64, 1), (256, 128, 2), (32, 512, 1), (512, 256, 3), (1024, 64, 1),
+                                             (64, 2048, 1), (2048, 32, 1), (1024, 1024, 2)])
+def test_repeated_solves_are_bitwise_reproducible(n_r, n_phi, batch):
+    """compute-sanitizer is closed on the GPU pool, so shared-memory hazards (the passes exchange through
+    shared memory under named barriers and mbarriers) are hunted this way: 12 repeats of the same solve,
+    enqueued back to back, must be identical bit for bit -- a race shows up as run-to-run differences."""
+    d = Dev(n_r, n_phi, 1.0, 300.0, 0.01, max_batch=batch)
+    try:
+        sig = torch.from_numpy(np.stack([random_sigma(n_r, n_phi, seed=700 + b, signed=True) for b in range(batch)])).cuda()
+        outs = [torch.empty_like(sig) for _ in range(12)]
+        for o in outs:
+            pg.pg_set_density(d.s.h, sig, batch, pg.PG_MEM_DEVICE)
+            pg.pg_potential(d.s.h, o, batch, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(d.s.h)
+        first = outs[0].cpu().numpy()
+        assert np.isfinite(first).all()
+        for k, o in enumerate(outs[1:], 1):
+            assert np.array_equal(o.cpu().numpy(), first), f"repeat {k} differs"
+    finally:
+        d.close()
