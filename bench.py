@@ -203,6 +203,8 @@ def run_ours(args):
     solver = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, max_batch=c.batch, device=local_rank,
                        cuda_stream=st.cuda_stream)
     h = solver.h
+    # the densities of the timed loop are resident in HBM and complete before the loop starts
+    pg.pg_set_option(h, pg.PG_OPT_DENSITY_STABLE, 1)
     r, phi, _ = solver.grid()
     n_fields = R * c.batch
     distinct = min(n_fields, 8 if c.n_r * c.n_phi >= 1 << 22 else 32)
@@ -319,6 +321,7 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
+                   "options": "PG_OPT_DENSITY_STABLE (densities resident and complete before the timed loop)",
                    "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
                          f"{R * pair_bytes / 1e6:.0f} MB in total vs 126 MB L2"},
         "cells_per_s": value * c.n_r * c.n_phi,

@@ -124,6 +124,18 @@ pg_status pg_grid(const pg_solver *s, double *r, double *phi, double *cell_area)
 
 /* Replace the (borrowed) stream; synchronises the old one first. */
 pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
+
+/* Options (off by default).
+ *   PG_OPT_DENSITY_STABLE  The caller promises that a PG_MEM_DEVICE density is complete in memory by the
+ *       time pg_potential is called: it is not being written by work still in flight on the stream (it was
+ *       produced before a synchronisation, or on another stream that has been joined).  The first forward
+ *       kernel may then fetch it while the previous kernel of the stream is still draining (programmatic
+ *       dependent launch; the library itself checks that it does not alias the potential its own previous
+ *       solve is still writing).  Time series and batches with densities resident in HBM (the case
+ *       bench.py times) qualify; a density written by the caller's kernel enqueued just before does not.
+ * Returns PG_ERR_INVALID_ARG for an unknown option. */
+typedef enum { PG_OPT_DENSITY_STABLE = 1 } pg_option;
+pg_status pg_set_option(pg_solver *s, pg_option option, int value);
 /* Block until all work enqueued by this solver has completed. */
 pg_status pg_synchronize(pg_solver *s);
 

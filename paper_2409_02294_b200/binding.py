@@ -18,12 +18,13 @@ PG_OK = 0
 PG_ERR_INVALID_ARG, PG_ERR_UNSUPPORTED, PG_ERR_CUDA, PG_ERR_NOMEM, PG_ERR_STATE = -1, -2, -3, -4, -5
 PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
 PG_NUM_KERNELS = 3
+PG_OPT_DENSITY_STABLE = 1
 KERNEL_NAMES = ("rows_fwd(a2)", "cols(a3+a4r)", "rows_inv(a4phi)")
 
 # every symbol include/polargrav.h declares
 EXPORTS = (
     "pg_create", "pg_create_ex", "pg_set_density", "pg_potential", "pg_potential_direct",
-    "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_synchronize",
+    "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_set_option", "pg_synchronize",
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
     "pg_version",
@@ -57,6 +58,7 @@ def lib():
         L.pg_destroy.argtypes = [vp]
         L.pg_grid.argtypes = [vp, vp, vp, vp]
         L.pg_set_stream.argtypes = [vp, vp]
+        L.pg_set_option.argtypes = [vp, i, i]
         L.pg_synchronize.argtypes = [vp]
         L.pg_host_alloc.argtypes = [ctypes.POINTER(vp), ctypes.c_size_t]
         L.pg_host_free.argtypes = [vp]
@@ -148,6 +150,10 @@ def pg_grid(h, n_r, n_phi):
 
 def pg_set_stream(h, cuda_stream):
     _check(lib().pg_set_stream(h, ctypes.c_void_p(cuda_stream) if cuda_stream else None), h)
+
+
+def pg_set_option(h, option, value):
+    _check(lib().pg_set_option(h, int(option), int(value)), h)
 
 
 def pg_synchronize(h):

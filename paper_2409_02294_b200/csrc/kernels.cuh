@@ -267,7 +267,7 @@ template <int NPHI>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
                 const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
-                const long w_field_stride)
+                const long w_field_stride, const int early_load)
 {
     typedef RowShape<NPHI> S;
     typedef Plan<S::L, ROW> P;
@@ -298,11 +298,14 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         cp_async_commit();
     };
 
-    // Sigma may come from the preceding kernel of the stream, and W is still read by it
+    // W is still read by the preceding kernel of the stream: nothing is stored before the wait.  Sigma
+    // is fetched ahead of it only when the host knows that no kernel that releases its dependents
+    // early (the library's own) writes it (polargrav.cu, early_load).
+    int item = blockIdx.x;
+    if (early_load && item < n_items) prefetch(item);
     pdl_wait();
     pdl_launch_dependents();
-    int item = blockIdx.x;
-    if (item < n_items) prefetch(item);
+    if (!early_load && item < n_items) prefetch(item);
     auto row_scale = [&](const int it) {
         return (rscale != nullptr && it < n_items) ? __ldg(&rscale[(it % items_per_field) * ROWS + rho]) : 1.0;
     };

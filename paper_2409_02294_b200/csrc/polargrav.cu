@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -55,6 +56,7 @@ struct pg_solver {
     const double *d_sigma = nullptr;
     int cur_batch = 0;
     bool sigma_from_host = false;
+    bool density_stable = false;   // PG_OPT_DENSITY_STABLE
 
     // host tables
     std::vector<double> r, phi, dA;
@@ -166,15 +168,37 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// Output range of the last kernel of this library that releases its dependents before it has
+// finished writing (rows_inv_kernel), per process: a rows_fwd_kernel launched right behind it may
+// read its input ahead of griddepcontrol.wait only if that input does not overlap this range.
+// (Any other producer of Sigma on the stream -- a copy, a kernel of the caller -- does not release
+// dependents early, so the launch itself is ordered behind its completion.)
+std::mutex g_out_mutex;
+const char *g_out_begin = nullptr, *g_out_end = nullptr;
+
+void note_early_release_output(const void *p, size_t bytes)
+{
+    std::lock_guard<std::mutex> lock(g_out_mutex);
+    g_out_begin = (const char *)p;
+    g_out_end = g_out_begin + bytes;
+}
+bool overlaps_early_release_output(const void *p, size_t bytes)
+{
+    std::lock_guard<std::mutex> lock(g_out_mutex);
+    const char *b = (const char *)p, *e = b + bytes;
+    return g_out_begin != nullptr && b < g_out_end && g_out_begin < e;
+}
+
 template <int NPHI>
 pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const double *rscale, int n_rows,
-                          int batch, long sigma_stride, long z_stride, cudaStream_t st)
+                          int batch, long sigma_stride, long z_stride, cudaStream_t st, bool early_ok)
 {
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (n_rows / S::ROWS) * batch;      // persistent CTAs walk over the items
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
     PG_CUDA(s, launch_pdl(pgk::rows_fwd_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, sigma, Z, s->d_tw_row,
-                          rscale, n_rows, n_items, sigma_stride, z_stride));
+                          rscale, n_rows, n_items, sigma_stride, z_stride,
+                          early_ok && !overlaps_early_release_output(sigma, (size_t)n_rows * NPHI * sizeof(double) * batch) ? 1 : 0));
     s->launches++;
     return PG_OK;
 }
@@ -188,6 +212,7 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
     PG_CUDA(s, launch_pdl(pgk::rows_inv_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, Z, phi, s->d_tw_row,
                           s->d_rs_out, s->n_r, n_items, z_stride, phi_stride));
+    note_early_release_output(phi, (size_t)s->n_r * NPHI * sizeof(double) * batch);
     s->launches++;
     return PG_OK;
 }
@@ -256,9 +281,9 @@ pg_status prepare_cols(pg_solver *s)
     }
 
 pg_status rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rscale, int n_rows, int batch,
-                   long sigma_stride, long w_stride, cudaStream_t st)
+                   long sigma_stride, long w_stride, cudaStream_t st, bool early_ok)
 {
-#define CALL(N) launch_rows_fwd<N>(s, sigma, W, rscale, n_rows, batch, sigma_stride, w_stride, st)
+#define CALL(N) launch_rows_fwd<N>(s, sigma, W, rscale, n_rows, batch, sigma_stride, w_stride, st, early_ok)
     PG_DISPATCH(s->n_phi, CALL)
 #undef CALL
 }
@@ -318,7 +343,7 @@ pg_status build_khat(pg_solver *s)
         s->launches++;
         if (cudaGetLastError() != cudaSuccess) { st = PG_ERR_CUDA; break; }
         // packed phi transform of the 2 n_r lag rows (no radial weight), transposed into ZK[k][2 n_r]
-        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream);
+        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream, false);
         if (st != PG_OK) break;
         // -G sinh(du) dphi (cell area / r^2), and the normalisation of the unnormalised transforms:
         // 1/(2 n_r) for the padded radial pair; 1/(2 n_phi) for the azimuthal pair (cols_kernel forms
@@ -384,7 +409,8 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         ev = &s->prof_pool[s->prof_used++];
         PG_CUDA(s, cudaEventRecord(ev->e[0], s->stream));
     }
-    pg_status st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream);
+    pg_status st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream,
+                            s->density_stable && !s->sigma_from_host);
     if (st != PG_OK) return st;
     if (ev) PG_CUDA(s, cudaEventRecord(ev->e[1], s->stream));
     st = cols(s, d_W, batch, ws, s->stream);
@@ -718,6 +744,16 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream)
     PG_CUDA(s, cudaStreamSynchronize(s->stream));
     s->stream = (cudaStream_t)cuda_stream;
     return PG_OK;
+}
+
+pg_status pg_set_option(pg_solver *s, pg_option option, int value)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    switch (option) {
+        case PG_OPT_DENSITY_STABLE: s->density_stable = value != 0; return PG_OK;
+    }
+    set_err(s, "pg_set_option: unknown option %d", (int)option);
+    return PG_ERR_INVALID_ARG;
 }
 
 pg_status pg_synchronize(pg_solver *s)

@@ -217,8 +217,9 @@ def test_zero_density_gives_zero_potential():
 
 
 # ---------------------------------------------------------------- the launch configuration bench.py times
+@pytest.mark.parametrize("stable", [0, 1])
 @pytest.mark.parametrize("cfg", [3, 5])
-def test_back_to_back_solves_equal_isolated_solves(cfg):
+def test_back_to_back_solves_equal_isolated_solves(cfg, stable):
     """bench.py enqueues solves back to back on one stream, rotating over distinct (Sigma, Phi) buffers,
     with the kernels chained by programmatic dependent launch (rows_fwd of solve n+1 is scheduled
     while rows_inv of solve n drains, and both use the one W workspace).  Every result of the chain
@@ -230,6 +231,7 @@ def test_back_to_back_solves_equal_isolated_solves(cfg):
         base = make_sigma(cfg, r, phi)
         fields = [np.ascontiguousarray(np.roll(base, 37 * k, axis=1) * (1.0 + 0.1 * k)) for k in range(6)]
         alone = [d.solve(f) for f in fields]
+        pg.pg_set_option(d.s.h, pg.PG_OPT_DENSITY_STABLE, stable)      # bench.py sets it
         d_s = [torch.from_numpy(f).cuda() for f in fields]
         d_p = [torch.empty_like(t) for t in d_s]
         torch.cuda.synchronize()
@@ -280,5 +282,28 @@ def test_repeated_solves_are_bitwise_reproducible(n_r, n_phi, batch):
         assert np.isfinite(first).all()
         for k, o in enumerate(outs[1:], 1):
             assert np.array_equal(o.cpu().numpy(), first), f"repeat {k} differs"
+    finally:
+        d.close()
+
+
+def test_potential_fed_back_as_density_with_early_fetch_enabled():
+    """PG_OPT_DENSITY_STABLE lets the first kernel of a solve fetch its input while the last kernel of the
+    previous solve is still draining.  If the caller (wrongly but plausibly) feeds the previous potential
+    straight back as the next density, the library must notice the aliasing and wait: the chain
+    Sigma -> Phi1 -> Phi2 -> Phi3 enqueued without synchronisation equals the synchronised one bit for bit."""
+    d = Dev(512, 2048, 1.0, 100.0, 0.01)
+    try:
+        s0 = random_sigma(512, 2048, seed=31)
+        p1 = d.solve(s0); p2 = d.solve(p1); p3 = d.solve(p2)
+        pg.pg_set_option(d.s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        bufs = [torch.from_numpy(s0).cuda()] + [torch.empty(512, 2048, dtype=torch.float64, device="cuda") for _ in range(3)]
+        torch.cuda.synchronize()
+        for rep in range(4):
+            for k in range(3):
+                pg.pg_set_density(d.s.h, bufs[k], 1, pg.PG_MEM_DEVICE)
+                pg.pg_potential(d.s.h, bufs[k + 1], 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(d.s.h)
+        for got, ref, name in zip(bufs[1:], (p1, p2, p3), ("Phi1", "Phi2", "Phi3")):
+            assert np.array_equal(got.cpu().numpy(), ref), name
     finally:
         d.close()
