@@ -462,11 +462,19 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     const Sync<T, S::THREADS> sync(ml + 1);
     fwd_a_compute_zero_upper<L, COL>(v, bases, u);
     fwd_a_store<L, COL>(v, line, u);
+    // Three-pass plans: pass B (in place) and pass C of a thread touch only slots of the 16 blocks
+    // 16 (u/16) .. 16 (u/16) + 15, i.e. the B <-> C exchanges stay inside aligned groups of 16 threads, and a
+    // warp-level barrier is enough for them.  Between the two CTA-wide barriers that are left the warps
+    // of a transform run free (pass B, pass C, multiply, inverse C, inverse B), so that the FP64 phases
+    // of some overlap the shared-memory phases of others.
+    static_assert(P::NPASS < 3 || (P::GB == 1 && P::MA == 16 * P::RC), "B <-> C exchange must stay inside 16-thread groups");
     if constexpr (P::NPASS == 3) {
         sync();
         fwd_b<L, COL>(line, bases, u);
+        __syncwarp();
+    } else {
+        sync();
     }
-    sync();
     fwd_c_col<L>(v, line, u);
     mbar_wait(kbar, 0);
 #pragma unroll
@@ -477,11 +485,11 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     }
     // inv_c writes exactly the 16 slots this thread has just read: no barrier in between
     inv_c_col<L>(v, line, u);
-    sync();
     if constexpr (P::NPASS == 3) {
+        __syncwarp();
         inv_b<L, COL>(line, bases, u);
-        sync();
     }
+    sync();
     inv_a_load<L, COL>(v, line, u);
     inv_a_compute_lower_half<L, COL>(v, bases, u);
     if (live) {
