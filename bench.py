@@ -373,6 +373,49 @@ NCU_FP64_INSTR: dict = {(5, 0): 0.97e8, (5, 1): 3.69e8, (5, 2): 0.97e8}
 FP64_LANES_PER_CLK_PER_SM = 64
 
 
+def run_direct(args):
+    """--direct: times the on-GPU cross-check (row a5, direct_kernel: tiled all-pairs summation from the
+    coordinates) on one field of the config and reports pair interactions per second.  Not the headline
+    metric and never a fallback; FP64-pipe bound."""
+    import torch
+    from paper_2409_02294_b200 import binding as pg, build as pg_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    c = CONFIGS[args.config]
+    st = torch.cuda.Stream()
+    solver = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, device=0, cuda_stream=st.cuda_stream)
+    r, phi, _ = solver.grid()
+    d_s = torch.from_numpy(make_sigma(args.config, r, phi, 0)).cuda()
+    d_p = torch.empty_like(d_s)
+    torch.cuda.synchronize()
+    rings = min(c.n_r, 296 if c.n_r * c.n_phi > 1 << 20 else c.n_r)     # bounded: a whole wave of target rings
+    steps = max(1, min(args.steps, 5))
+
+    def step():
+        pg.pg_set_density(solver.h, d_s, 1, pg.PG_MEM_DEVICE)
+        pg.pg_potential_direct_rings(solver.h, d_p, 0, rings, pg.PG_MEM_DEVICE)
+
+    step(); pg.pg_synchronize(solver.h)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(steps):
+        step()
+    e1.record(st)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    pairs = float(rings) * c.n_phi * c.n_r * c.n_phi
+    line = {"metric": "pair interactions/sec (fp64 direct summation cross-check, row a5)", "value": pairs / (ms * 1e-3),
+            "unit": "pairs/s", "n_gpus": 1, "steps": steps, "warmup": 1, "ms_per_step": ms, "higher_is_better": True,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "target_rings": rings, "pairs_per_step": pairs},
+            "extrapolated_full_grid_s": ms * 1e-3 * c.n_r / rings}
+    solver.close()
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -381,7 +424,10 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     args = ap.parse_args()
+    if args.direct:
+        return run_direct(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)

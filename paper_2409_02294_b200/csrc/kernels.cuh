@@ -612,4 +612,95 @@ direct_kernel(const double *__restrict__ sigma, double *__restrict__ phi, const 
     }
 }
 
+// Register-tiled variant for n_phi >= 256.  For one ring pair the sum over j' is a cyclic correlation of the
+// source ring w[j'] with the pair kernel g[(j - j') mod n_phi]: a thread that owns R CONSECUTIVE targets
+// j0 .. j0+R-1 and walks over the sources in blocks of 8 needs, per block, 8 values of w and the R + 7 kernel
+// values of the lags j0 - j'0 - 7 .. j0 - j'0 + R - 1 -- a window that slides down by 8 from block to block, so
+// that only 8 new values are loaded per block: 8 R FMAs for 8 + 8 shared-memory doubles, against two loads per
+// FMA in direct_kernel.  The kernel is stored twice over (lags 0 .. 2 n_phi - 1) so that a window never wraps,
+// in groups of R padded to R + 2 doubles (lane stride an odd number of 16-byte units: conflict-free loads).  Same arithmetic per
+// pair and the same two-level accumulation as direct_kernel; the summation order within a ring differs.
+template <int R>
+__global__ void __launch_bounds__(128)
+direct_tiled_kernel(const double *__restrict__ sigma, double *__restrict__ phi, const double *__restrict__ r,
+                    const double *__restrict__ dA, const double *__restrict__ s2, const int n_r, const int n_phi,
+                    const double eps2, const int ring0, const long sigma_field_stride, const long phi_field_stride)
+{
+    static_assert(R % 8 == 0 && R >= 8 && R <= 16, "targets per thread");
+    constexpr int NG = R / 8 + 1;                       // groups of 8 lags in the window
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *w = reinterpret_cast<double *>(smem_raw);   // [n_phi] Sigma of the source ring
+    double *g = w + n_phi;                              // [2 n_phi / R][R + 2] pair kernel by lag, twice over
+    auto slot = [](const int lag) { return (lag / R) * (R + 2) + lag % R; };
+    const int i = ring0 + blockIdx.x;
+    const double ri = r[i], hi = sqrt(dA[i]);
+    const double *sg = sigma + blockIdx.y * sigma_field_stride;
+    const int nt = blockDim.x;
+    const int j0 = R * threadIdx.x;
+
+    double acc[R];
+#pragma unroll
+    for (int q = 0; q < R; ++q) acc[q] = 0.0;
+
+    for (int ip = 0; ip < n_r; ++ip) {
+        const double rp = r[ip], ap = dA[ip];
+        const double dr = ri - rp;
+        const double base = fma(dr, dr, eps2 * hi * sqrt(ap));
+        const double rr4 = 4.0 * ri * rp;
+        __syncthreads();
+        for (int l = threadIdx.x; l < n_phi; l += nt) {
+            w[l] = sg[(long)ip * n_phi + l];
+            const double gv = rsqrt(fma(rr4, s2[l], base));
+            g[slot(l)] = gv;
+            g[slot(l + n_phi)] = gv;
+        }
+        __syncthreads();
+        double ring[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) ring[q] = 0.0;
+        // window gw[k] = g_ext[n_phi + j0 - jp0 - 8 + k], k < 8 NG; target j0 + q, source jp0 + t: lag index q - t + 8
+        double gw[8 * NG];
+        const int lag0 = n_phi + j0 - 8;                     // first lag of the window for jp0 = 0
+#pragma unroll
+        for (int k = 1; k < NG; ++k) {                       // groups above the lowest one, for jp0 = 0
+            const double2 *gp = reinterpret_cast<const double2 *>(g + slot(lag0 + 8 * k));
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const double2 t2 = gp[h];
+                gw[8 * k + 2 * h] = t2.x;
+                gw[8 * k + 2 * h + 1] = t2.y;
+            }
+        }
+        for (int jp0 = 0; jp0 < n_phi; jp0 += 8) {
+            const double2 *gp = reinterpret_cast<const double2 *>(g + slot(lag0 - jp0));
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const double2 t2 = gp[h];
+                gw[2 * h] = t2.x;
+                gw[2 * h + 1] = t2.y;
+            }
+            const double2 *wp = reinterpret_cast<const double2 *>(w + jp0);
+            double wv[8];
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                const double2 t2 = wp[h];
+                wv[2 * h] = t2.x;
+                wv[2 * h + 1] = t2.y;
+            }
+#pragma unroll
+            for (int t = 0; t < 8; ++t)
+#pragma unroll
+                for (int q = 0; q < R; ++q) ring[q] = fma(wv[t], gw[q - t + 8], ring[q]);
+            // slide the window: the groups move up by one
+#pragma unroll
+            for (int k = 8 * NG - 1; k >= 8; --k) gw[k] = gw[k - 8];
+        }
+#pragma unroll
+        for (int q = 0; q < R; ++q) acc[q] = fma(ap, ring[q], acc[q]);
+    }
+    double *out = phi + blockIdx.y * phi_field_stride + (long)blockIdx.x * n_phi + j0;
+#pragma unroll
+    for (int q = 0; q < R; ++q) out[q] = -acc[q];
+}
+
 }  // namespace pgk

@@ -424,6 +424,25 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
 
 pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int ring0, int n_rings, int batch)
 {
+    if (s->n_phi >= 256) {
+        // register-tiled kernel: 16 consecutive targets per thread (8 below 1024), Sigma ring + doubled, padded kernel
+        const int R = s->n_phi >= 1024 ? 16 : 8;
+        const size_t smem = ((size_t)s->n_phi + (size_t)(2 * s->n_phi / R) * (R + 2)) * sizeof(double);
+        const double eps2 = s->eps * s->eps;
+        dim3 grid(n_rings, batch);
+        const long fs = (long)s->field;
+        if (s->n_phi >= 1024) {
+            PG_CUDA(s, cudaFuncSetAttribute(pgk::direct_tiled_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            pgk::direct_tiled_kernel<16><<<grid, s->n_phi / 16, smem, s->stream>>>(d_sigma, d_phi, s->d_r, s->d_dA, s->d_s2, s->n_r,
+                                                                                   s->n_phi, eps2, ring0, fs, fs);
+        } else {
+            pgk::direct_tiled_kernel<8><<<grid, s->n_phi / 8, smem, s->stream>>>(d_sigma, d_phi, s->d_r, s->d_dA, s->d_s2, s->n_r,
+                                                                                 s->n_phi, eps2, ring0, fs, fs);
+        }
+        PG_CUDA(s, cudaGetLastError());
+        s->launches++;
+        return PG_OK;
+    }
     const int threads = s->n_phi < 256 ? s->n_phi : 256;
     const int tpt = s->n_phi / threads;
     const size_t smem = 2 * (size_t)s->n_phi * sizeof(double);
