@@ -390,7 +390,7 @@ def run_direct(args):
     d_s = torch.from_numpy(make_sigma(args.config, r, phi, 0)).cuda()
     d_p = torch.empty_like(d_s)
     torch.cuda.synchronize()
-    rings = min(c.n_r, 296 if c.n_r * c.n_phi > 1 << 20 else c.n_r)     # bounded: a whole wave of target rings
+    rings = min(c.n_r, 888 if c.n_r * c.n_phi > 1 << 20 else c.n_r)     # bounded: two full waves of target rings (3 CTAs per SM)
     steps = max(1, min(args.steps, 5))
 
     def step():
