@@ -106,32 +106,10 @@ __device__ __forceinline__ cplx mulroot(cplx z)
 }
 
 // ------------------------------------------------------------------ radix-N DFT in registers
-// In-place decimation-in-frequency on x[0..N): output X[k] lands at slot bitrev(k).
-template <int N, bool INV, int J = 0>
-struct DifStage {
-    static __device__ __forceinline__ void run(cplx *x)
-    {
-        if constexpr (J < N / 2) {
-            const cplx a = x[J], b = x[J + N / 2];
-            x[J] = cadd(a, b);
-            x[J + N / 2] = mulroot<J * (32 / N), INV>(csub(a, b));
-            DifStage<N, INV, J + 1>::run(x);
-        }
-    }
-};
-
-template <int N, bool INV>
-struct Dif {
-    static __device__ __forceinline__ void run(cplx *x)
-    {
-        if constexpr (N >= 2) {
-            DifStage<N, INV>::run(x);
-            Dif<N / 2, INV>::run(x);
-            Dif<N / 2, INV>::run(x + N / 2);
-        }
-    }
-};
-
+// Decimation in time on bit-reversed inputs.  A butterfly (a, b) -> (a + w b, a - w b) with a non-trivial
+// constant root w = c (1 + i t) costs 6 FMAs instead of a 4-instruction product and 4 additions:
+//   u = b.x - t b.y,  v = b.y + t b.x,   a +- c (u, v).
+// A radix-16 DFT is then 148 FP64 instructions instead of 168 (all of them occupy the same pipe).
 template <int N>
 __host__ __device__ constexpr int bitrev(int k)
 {
@@ -140,15 +118,60 @@ __host__ __device__ constexpr int bitrev(int k)
     return r;
 }
 
+// (a, b) <- (a + w b, a - w b),  w = exp(-/+ 2 pi i NUM / 32)   (- forward, + inverse),  0 <= NUM < 16
+template <int NUM, bool INV>
+__device__ __forceinline__ void butterfly(cplx &a, cplx &b)
+{
+    static_assert(NUM >= 0 && NUM < 16, "root");
+    if constexpr (NUM == 0) {
+        const cplx s = cadd(a, b), d = csub(a, b);
+        a = s; b = d;
+    } else if constexpr (NUM == 8) {        // w = -i (forward), +i (inverse)
+        const cplx wb = INV ? make_double2(-b.y, b.x) : make_double2(b.y, -b.x);
+        const cplx s = cadd(a, wb), d = csub(a, wb);
+        a = s; b = d;
+    } else {
+        constexpr double c = cos32(NUM);
+        constexpr double t = (INV ? sin32(NUM) : -sin32(NUM)) / cos32(NUM);
+        const double u = fma(-t, b.y, b.x);
+        const double v = fma(t, b.x, b.y);
+        const cplx s = make_double2(fma(c, u, a.x), fma(c, v, a.y));
+        const cplx d = make_double2(fma(-c, u, a.x), fma(-c, v, a.y));
+        a = s; b = d;
+    }
+}
+// the butterflies of the stage that merges blocks of LEN/2 into blocks of LEN
+template <int N, int LEN, bool INV, int B = 0, int J = 0>
+__device__ __forceinline__ void dit_stage(cplx *y)
+{
+    if constexpr (B < N) {
+        if constexpr (J < LEN / 2) {
+            butterfly<J * (32 / LEN), INV>(y[B + J], y[B + J + LEN / 2]);
+            dit_stage<N, LEN, INV, B, J + 1>(y);
+        } else {
+            dit_stage<N, LEN, INV, B + LEN, 0>(y);
+        }
+    }
+}
+template <int N, int LEN, bool INV>
+__device__ __forceinline__ void dit_stages(cplx *y)
+{
+    if constexpr (LEN <= N) {
+        dit_stage<N, LEN, INV>(y);
+        dit_stages<N, 2 * LEN, INV>(y);
+    }
+}
+
 // natural order in -> natural order out (x is any array of at least N elements)
 template <int N, bool INV>
 __device__ __forceinline__ void dft(cplx *x)
 {
+    static_assert(N <= 32, "radix");
     if constexpr (N >= 2) {
-        Dif<N, INV>::run(x);
         cplx y[N];
 #pragma unroll
         for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
+        dit_stages<N, 2, INV>(y);
 #pragma unroll
         for (int k = 0; k < N; ++k) x[k] = y[k];
     }
@@ -169,12 +192,12 @@ template <int N>
 __device__ __forceinline__ void dft_zero_upper(cplx *x)
 {
     static_assert(N >= 2 && N <= 32, "radix");
-    zero_upper_stage<N>(x);
-    Dif<N / 2, false>::run(x);
-    Dif<N / 2, false>::run(x + N / 2);
+    zero_upper_stage<N>(x);                 // even bins: DFT of x[0..N/2); odd bins: DFT of the rotated copy
+    dft<N / 2, false>(x);
+    dft<N / 2, false>(x + N / 2);
     cplx y[N];
 #pragma unroll
-    for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
+    for (int k = 0; k < N / 2; ++k) { y[2 * k] = x[k]; y[2 * k + 1] = x[N / 2 + k]; }
 #pragma unroll
     for (int k = 0; k < N; ++k) x[k] = y[k];
 }
