@@ -362,14 +362,14 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/), keyed by (config, kernel index).  Filled in from profiles/*.md; None = not captured.
-NCU_TRAFFIC: dict = {          # profiles/r1_04_final.md
-    (5, 0): 33.6e6 + 1.0e6,    # rows_fwd_kernel<2048>
-    (5, 1): 67.2e6 + 0.9e6,    # cols_kernel<2048>
-    (5, 2): 33.6e6 + 0.5e6,    # rows_inv_kernel<2048>
+NCU_TRAFFIC: dict = {          # profiles/r1_06_end_of_round.md
+    (5, 0): 33.6e6 + 0.9e6,    # rows_fwd_kernel<2048>
+    (5, 1): 67.2e6 + 1.0e6,    # cols_kernel<2048>
+    (5, 2): 33.6e6 + 0.4e6,    # rows_inv_kernel<2048>
 }
 # FP64 thread instructions (DADD + DMUL + DFMA) per launch from the same capture; the FP64 pipe issues
 # 64 per clock per SM (ncu sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained)
-NCU_FP64_INSTR: dict = {(5, 0): 0.97e8, (5, 1): 3.69e8, (5, 2): 0.97e8}
+NCU_FP64_INSTR: dict = {(5, 0): 0.93e8, (5, 1): 3.51e8, (5, 2): 0.93e8}
 FP64_LANES_PER_CLK_PER_SM = 64
 
 
