@@ -131,8 +131,11 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
  *       produced before a synchronisation, or on another stream that has been joined).  The first forward
  *       kernel may then fetch it while the previous kernel of the stream is still draining (programmatic
  *       dependent launch; the library itself checks that it does not alias the potential its own previous
- *       solve is still writing).  Time series and batches with densities resident in HBM (the case
- *       bench.py times) qualify; a density written by the caller's kernel enqueued just before does not.
+ *       solve is still writing), and, working alternately in two copies of its intermediate spectrum
+ *       (a second workspace of max_batch * (n_phi/2 + 1) * n_r * 16 bytes is allocated on first use), runs
+ *       entirely alongside the tail of the previous solve's last kernel.  Time series and batches with
+ *       densities resident in HBM (the case bench.py times) qualify; a density written by the caller's
+ *       kernel enqueued just before does not.
  * Returns PG_ERR_INVALID_ARG for an unknown option. */
 typedef enum { PG_OPT_DENSITY_STABLE = 1 } pg_option;
 pg_status pg_set_option(pg_solver *s, pg_option option, int value);

@@ -298,12 +298,17 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         cp_async_commit();
     };
 
-    // W is still read by the preceding kernel of the stream: nothing is stored before the wait.  Sigma
-    // is fetched ahead of it only when the host knows that no kernel that releases its dependents
-    // early (the library's own) writes it (polargrav.cu, early_load).
+    // Dependence on the preceding kernel of the stream (polargrav.cu decides, `early_load`):
+    //   0  Sigma may be its output, and it may still read W: wait before anything else.
+    //   1  Sigma is known to be complete, W is the buffer the preceding kernel reads: the first item is
+    //      fetched ahead of the wait, nothing is stored before it.
+    //   2  Sigma is complete AND W is a buffer no kernel in flight touches (the solver alternates between
+    //      two): this kernel depends on nothing that runs before it.  It does all its work at once --
+    //      filling the SMs the preceding kernel leaves idle in its last, uneven round -- and waits at its
+    //      END, so that its own completion still implies that of everything before it.
     int item = blockIdx.x;
     if (early_load && item < n_items) prefetch(item);
-    pdl_wait();
+    if (early_load < 2) pdl_wait();
     pdl_launch_dependents();
     if (!early_load && item < n_items) prefetch(item);
     auto row_scale = [&](const int it) {
@@ -338,6 +343,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         else split_special<L>(v, un1, un2, store);
         __syncthreads();   // the lines are rewritten by the next item's pass A
     }
+    if (early_load == 2) pdl_wait();
 }
 
 // ---------------------------------------------------------------- a4 (phi part): rows inverse

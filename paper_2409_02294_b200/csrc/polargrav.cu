@@ -43,6 +43,8 @@ struct pg_solver {
 
     // device memory (owned)
     cplx *d_W = nullptr;          // W: [max_batch][half+1][n_r]
+    cplx *d_W_alt = nullptr;      // second W (lazily allocated): resident solves alternate, see solve_fields
+    const cplx *last_w = nullptr; // the W buffer the most recent solve of this solver works in
     double *d_khat = nullptr;     // [half+1][2][n_r]
     cplx *d_tw_row = nullptr;     // Plan<n_phi/2, ROW> twiddle table
     cplx *d_tw_col = nullptr;     // Plan<2 n_r, COL> twiddle table
@@ -191,14 +193,14 @@ bool overlaps_early_release_output(const void *p, size_t bytes)
 
 template <int NPHI>
 pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const double *rscale, int n_rows,
-                          int batch, long sigma_stride, long z_stride, cudaStream_t st, bool early_ok)
+                          int batch, long sigma_stride, long z_stride, cudaStream_t st, int early_mode)
 {
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (n_rows / S::ROWS) * batch;      // persistent CTAs walk over the items
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
     PG_CUDA(s, launch_pdl(pgk::rows_fwd_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, sigma, Z, s->d_tw_row,
                           rscale, n_rows, n_items, sigma_stride, z_stride,
-                          early_ok && !overlaps_early_release_output(sigma, (size_t)n_rows * NPHI * sizeof(double) * batch) ? 1 : 0));
+                          early_mode));
     s->launches++;
     return PG_OK;
 }
@@ -281,9 +283,9 @@ pg_status prepare_cols(pg_solver *s)
     }
 
 pg_status rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rscale, int n_rows, int batch,
-                   long sigma_stride, long w_stride, cudaStream_t st, bool early_ok)
+                   long sigma_stride, long w_stride, cudaStream_t st, int early_mode)
 {
-#define CALL(N) launch_rows_fwd<N>(s, sigma, W, rscale, n_rows, batch, sigma_stride, w_stride, st, early_ok)
+#define CALL(N) launch_rows_fwd<N>(s, sigma, W, rscale, n_rows, batch, sigma_stride, w_stride, st, early_mode)
     PG_DISPATCH(s->n_phi, CALL)
 #undef CALL
 }
@@ -343,7 +345,7 @@ pg_status build_khat(pg_solver *s)
         s->launches++;
         if (cudaGetLastError() != cudaSuccess) { st = PG_ERR_CUDA; break; }
         // packed phi transform of the 2 n_r lag rows (no radial weight), transposed into ZK[k][2 n_r]
-        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream, false);
+        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream, 0);
         if (st != PG_OK) break;
         // -G sinh(du) dphi (cell area / r^2), and the normalisation of the unnormalised transforms:
         // 1/(2 n_r) for the padded radial pair; 1/(2 n_phi) for the azimuthal pair (cols_kernel forms
@@ -409,8 +411,26 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         ev = &s->prof_pool[s->prof_used++];
         PG_CUDA(s, cudaEventRecord(ev->e[0], s->stream));
     }
-    pg_status st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream,
-                            s->density_stable && !s->sigma_from_host);
+    // How much rows_fwd depends on the kernel before it (kernels.cuh): with a stable density that does not
+    // alias the potential still being written, the first item is fetched early (1); if the solve also
+    // works in the W buffer the previous solve did not use, it depends on nothing in flight (2).
+    int early = 0;
+    if (s->density_stable && !s->sigma_from_host &&
+        !overlaps_early_release_output(d_sigma, (size_t)batch * s->field * sizeof(double))) {
+        early = 1;
+        if (d_W == s->d_W && !ev) {
+            if (!s->d_W_alt) {
+                const size_t w_bytes = (size_t)s->max_batch * (s->half + 1) * s->n_r * sizeof(cplx);
+                if (cudaMalloc((void **)&s->d_W_alt, w_bytes) != cudaSuccess) { s->d_W_alt = nullptr; (void)cudaGetLastError(); }
+            }
+            if (s->d_W_alt) {
+                d_W = (s->last_w == s->d_W) ? s->d_W_alt : s->d_W;     // the one the previous solve does not use
+                early = 2;
+            }
+        }
+    }
+    s->last_w = (d_W == s->d_W_alt) ? s->d_W_alt : s->d_W;
+    pg_status st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream, early);
     if (st != PG_OK) return st;
     if (ev) PG_CUDA(s, cudaEventRecord(ev->e[1], s->stream));
     st = cols(s, d_W, batch, ws, s->stream);
@@ -468,7 +488,7 @@ pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int 
 void free_all(pg_solver *s)
 {
     if (!s) return;
-    cudaFree(s->d_W); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_tw_col);
+    cudaFree(s->d_W); cudaFree(s->d_W_alt); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_tw_col);
     cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
     cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); cudaFree(s->d_sigma_own); cudaFree(s->d_phi_own);
     if (s->h_in) cudaFreeHost(s->h_in);
