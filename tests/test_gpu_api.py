@@ -111,8 +111,13 @@ def test_state_and_argument_errors(solver):
         pg.pg_potential(solver.h, out, 2, pg.PG_MEM_HOST)           # batch mismatch
     assert e.value.status == pg.PG_ERR_INVALID_ARG
     assert "batch" in pg.last_error(solver.h)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_set_option(solver.h, 99, 1)                           # unknown option
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    pg.pg_set_option(solver.h, pg.PG_OPT_DENSITY_STABLE, 1)         # has no effect on host-staged solves
     pg.pg_potential(solver.h, out, 1, pg.PG_MEM_HOST)               # still usable after errors
     assert np.isfinite(out).all()
+    pg.pg_set_option(solver.h, pg.PG_OPT_DENSITY_STABLE, 0)
 
 
 def test_nan_propagates_not_checked(solver):

@@ -307,3 +307,34 @@ def test_potential_fed_back_as_density_with_early_fetch_enabled():
             assert np.array_equal(got.cpu().numpy(), ref), name
     finally:
         d.close()
+
+
+def test_resident_and_staged_solves_interleaved_with_the_option_on():
+    """With PG_OPT_DENSITY_STABLE the solver alternates between two W buffers and lets the forward row kernel
+    run ahead of the previous solve's last kernel; host-staged solves always use the first buffer and wait.
+    Any interleaving of the two kinds, enqueued without synchronisation, must reproduce the isolated results."""
+    d = Dev(1024, 512, 1.0, 300.0, 0.01)
+    try:
+        fields = [random_sigma(1024, 512, seed=40 + k) for k in range(5)]
+        alone = [d.solve(f) for f in fields]
+        pg.pg_set_option(d.s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        d_s = [torch.from_numpy(f).cuda() for f in fields]
+        d_p = [torch.empty_like(t) for t in d_s]
+        pin_in, pin_out = pg.PinnedArray((1024, 512)), pg.PinnedArray((1024, 512))
+        pin_in.array[...] = fields[4]
+        torch.cuda.synchronize()
+        pattern = [0, 1, "host", 2, "host", "host", 3, 0, 1, "host", 2, 3]
+        for what in pattern:
+            if what == "host":
+                pg.pg_set_density(d.s.h, pin_in.ptr, 1, pg.PG_MEM_HOST_PINNED)
+                pg.pg_potential(d.s.h, pin_out.ptr, 1, pg.PG_MEM_HOST_PINNED)
+            else:
+                pg.pg_set_density(d.s.h, d_s[what], 1, pg.PG_MEM_DEVICE)
+                pg.pg_potential(d.s.h, d_p[what], 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(d.s.h)
+        for k in range(4):
+            assert np.array_equal(d_p[k].cpu().numpy(), alone[k]), f"resident field {k}"
+        assert np.array_equal(pin_out.array, alone[4]), "host-staged field"
+        pin_in.free(); pin_out.free()
+    finally:
+        d.close()
