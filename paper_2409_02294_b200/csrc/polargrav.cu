@@ -50,7 +50,13 @@ struct pg_solver {
     cplx *d_tw_col = nullptr;     // Plan<2 n_r, COL> twiddle table
     double *d_rs_in = nullptr, *d_rs_out = nullptr;
     double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
-    double *d_sigma_own = nullptr, *d_phi_own = nullptr;   // [max_batch][n_r][n_phi], lazily allocated
+    // [max_batch][n_r][n_phi] each, lazily allocated, TWO slots per direction: the upload of the next
+    // density does not wait for the solve that still reads the previous one, and a solve does not wait for
+    // the download of the previous potential
+    double *d_sigma_own[2] = {nullptr, nullptr}, *d_phi_own[2] = {nullptr, nullptr};
+    int in_slot = 0, out_slot = 0;
+    cudaEvent_t ev_in_free[2] = {nullptr, nullptr};    // main stream: the solves reading sigma slot k are done
+    cudaEvent_t ev_out_done[2] = {nullptr, nullptr};   // d2h stream: the downloads from phi slot k are done
     // pinned host staging (owned, lazily allocated)
     double *h_in = nullptr, *h_out = nullptr;
 
@@ -365,8 +371,10 @@ pg_status build_khat(pg_solver *s)
 pg_status ensure_staging(pg_solver *s, bool need_in, bool need_out)
 {
     const size_t bytes = s->field * (size_t)s->max_batch * sizeof(double);
-    if (need_in && !s->d_sigma_own) PG_CUDA(s, cudaMalloc((void **)&s->d_sigma_own, bytes));
-    if (need_out && !s->d_phi_own) PG_CUDA(s, cudaMalloc((void **)&s->d_phi_own, bytes));
+    for (int k = 0; k < 2; ++k) {
+        if (need_in && !s->d_sigma_own[k]) PG_CUDA(s, cudaMalloc((void **)&s->d_sigma_own[k], bytes));
+        if (need_out && !s->d_phi_own[k]) PG_CUDA(s, cudaMalloc((void **)&s->d_phi_own[k], bytes));
+    }
     return PG_OK;
 }
 pg_status ensure_pinned(pg_solver *s, bool in, bool out)
@@ -490,7 +498,12 @@ void free_all(pg_solver *s)
     if (!s) return;
     cudaFree(s->d_W); cudaFree(s->d_W_alt); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_tw_col);
     cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
-    cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); cudaFree(s->d_sigma_own); cudaFree(s->d_phi_own);
+    cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); 
+    for (int k = 0; k < 2; ++k) {
+        cudaFree(s->d_sigma_own[k]); cudaFree(s->d_phi_own[k]);
+        if (s->ev_in_free[k]) cudaEventDestroy(s->ev_in_free[k]);
+        if (s->ev_out_done[k]) cudaEventDestroy(s->ev_out_done[k]);
+    }
     if (s->h_in) cudaFreeHost(s->h_in);
     if (s->h_out) cudaFreeHost(s->h_out);
     for (auto e : s->ev_in) if (e) cudaEventDestroy(e);
@@ -577,6 +590,10 @@ pg_status create_impl(pg_solver *s)
         PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_out[b], cudaEventDisableTiming));
     }
     PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_main, cudaEventDisableTiming));
+    for (int k = 0; k < 2; ++k) {
+        PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_in_free[k], cudaEventDisableTiming));
+        PG_CUDA(s, cudaEventCreateWithFlags(&s->ev_out_done[k], cudaEventDisableTiming));
+    }
 
     if ((st = prepare_kernels_rows(s)) != PG_OK) return st;
     if ((st = prepare_kernels_cols(s)) != PG_OK) return st;
@@ -651,9 +668,10 @@ pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspa
         pg_status st = ensure_staging(s, true, false);
         if (st != PG_OK) return st;
         if (where == PG_MEM_HOST && (st = ensure_pinned(s, true, false)) != PG_OK) return st;
-        // the owned device copy may still be read by solves already enqueued on the main stream
-        PG_CUDA(s, cudaEventRecord(s->ev_main, s->stream));
-        PG_CUDA(s, cudaStreamWaitEvent(s->h2d, s->ev_main, 0));
+        // the other staging slot: only the solves that read THAT one (two densities ago) must be done
+        s->in_slot ^= 1;
+        double *d_own = s->d_sigma_own[s->in_slot];
+        PG_CUDA(s, cudaStreamWaitEvent(s->h2d, s->ev_in_free[s->in_slot], 0));
         for (int b = 0; b < batch; ++b) {
             const double *src = sigma + (size_t)b * s->field;
             if (where == PG_MEM_HOST) {
@@ -662,12 +680,11 @@ pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspa
                 memcpy(stage, src, fbytes);
                 src = stage;
             }
-            PG_CUDA(s, cudaMemcpyAsync(s->d_sigma_own + (size_t)b * s->field, src, fbytes, cudaMemcpyHostToDevice,
-                                       s->h2d));
+            PG_CUDA(s, cudaMemcpyAsync(d_own + (size_t)b * s->field, src, fbytes, cudaMemcpyHostToDevice, s->h2d));
             PG_CUDA(s, cudaEventRecord(s->ev_in[b], s->h2d));
             s->in_pending[b] = 1;
         }
-        s->d_sigma = s->d_sigma_own;
+        s->d_sigma = d_own;
         s->sigma_from_host = true;
     } else {
         set_err(s, "pg_set_density: unknown memspace %d", (int)where);
@@ -714,15 +731,17 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
 
     // staged pipeline: field b is solved as soon as its H2D copy has landed, and copied back
     // while field b+1 is being solved (copy streams h2d / d2h, compute on the caller's stream)
+    double *d_out = nullptr;
     if (host_out) {
-        // previous D2H copies read d_phi_own
-        PG_CUDA(s, cudaEventRecord(s->ev_main, s->d2h));
-        PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_main, 0));
+        // the other staging slot: only the downloads from THAT one (two potentials ago) must be done
+        s->out_slot ^= 1;
+        d_out = s->d_phi_own[s->out_slot];
+        PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_out_done[s->out_slot], 0));
     }
     for (int b = 0; b < batch; ++b) {
         if (s->sigma_from_host) PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_in[b], 0));
         const double *sg = s->d_sigma + (size_t)b * s->field;
-        double *dst = host_out ? s->d_phi_own + (size_t)b * s->field : phi + (size_t)b * out_field;
+        double *dst = host_out ? d_out + (size_t)b * s->field : phi + (size_t)b * out_field;
         if (direct) st = launch_direct(s, sg, dst, rings ? ring0 : 0, rings ? n_rings : s->n_r, 1);
         else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * (s->half + 1) * s->n_r, 1);
         if (st != PG_OK) return st;
@@ -734,6 +753,8 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
             PG_CUDA(s, cudaEventRecord(s->ev_out[b], s->d2h));
         }
     }
+    if (host_out) PG_CUDA(s, cudaEventRecord(s->ev_out_done[s->out_slot], s->d2h));
+    if (s->sigma_from_host) PG_CUDA(s, cudaEventRecord(s->ev_in_free[s->in_slot], s->stream));
     if (where == PG_MEM_HOST) {
         for (int b = 0; b < batch; ++b) {
             PG_CUDA(s, cudaEventSynchronize(s->ev_out[b]));
