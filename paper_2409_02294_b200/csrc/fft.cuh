@@ -162,6 +162,16 @@ __device__ __forceinline__ void dit_stages(cplx *y)
     }
 }
 
+// the stages LEN, 2 LEN, ..., LAST only
+template <int N, int LEN, int LAST, bool INV>
+__device__ __forceinline__ void dit_stages_upto(cplx *y)
+{
+    if constexpr (LEN <= LAST) {
+        dit_stage<N, LEN, INV>(y);
+        dit_stages_upto<N, 2 * LEN, LAST, INV>(y);
+    }
+}
+
 // natural order in -> natural order out (x is any array of at least N elements)
 template <int N, bool INV>
 __device__ __forceinline__ void dft(cplx *x)
@@ -178,49 +188,58 @@ __device__ __forceinline__ void dft(cplx *x)
 }
 
 // ------------------------------------------------------------------ pruned radix-N DFTs (zero-padded transforms)
-// Forward DFT of N points whose upper half is zero: x[0..N/2) in, X[0..N) out (natural order).
-// The first decimation-in-frequency stage degenerates to a copy and a rotation.
-template <int N, int J = 0>
-__device__ __forceinline__ void zero_upper_stage(cplx *x)
-{
-    if constexpr (J < N / 2) {
-        x[J + N / 2] = mulroot<J * (32 / N), false>(x[J]);
-        zero_upper_stage<N, J + 1>(x);
-    }
-}
+// Forward DFT of N points whose upper half is zero: x[0..N/2) in, X[0..N) out (natural order).  In the
+// bit-reversed input order of the decimation-in-time flow the zeros are the odd positions, so the first stage
+// degenerates to copies.
 template <int N>
 __device__ __forceinline__ void dft_zero_upper(cplx *x)
 {
     static_assert(N >= 2 && N <= 32, "radix");
-    zero_upper_stage<N>(x);                 // even bins: DFT of x[0..N/2); odd bins: DFT of the rotated copy
-    dft<N / 2, false>(x);
-    dft<N / 2, false>(x + N / 2);
     cplx y[N];
 #pragma unroll
-    for (int k = 0; k < N / 2; ++k) { y[2 * k] = x[k]; y[2 * k + 1] = x[N / 2 + k]; }
+    for (int j = 0; j < N / 2; ++j) y[2 * j] = y[2 * j + 1] = x[bitrev<N>(2 * j)];
+    dit_stages<N, 4, false>(y);
 #pragma unroll
     for (int k = 0; k < N; ++k) x[k] = y[k];
 }
-// Inverse DFT of N points of which only the lower half of the outputs is wanted:
-// y[n] = sum_d X[d] exp(+2 pi i n d / N), n < N/2, left in x[0..N/2)  (decimation in time, last stage halved)
-template <int N, int K = 0>
-__device__ __forceinline__ void lower_half_stage(cplx *x, const cplx *e, const cplx *o)
+// a <- a + w b,  w = exp(-/+ 2 pi i NUM / 32): the half of a butterfly whose other output is not wanted
+template <int NUM, bool INV>
+__device__ __forceinline__ void half_butterfly(cplx &a, const cplx b)
 {
-    if constexpr (K < N / 2) {
-        x[K] = cadd(e[K], mulroot<K * (32 / N), true>(o[K]));
-        lower_half_stage<N, K + 1>(x, e, o);
+    static_assert(NUM >= 0 && NUM < 16, "root");
+    if constexpr (NUM == 0) {
+        a = cadd(a, b);
+    } else if constexpr (NUM == 8) {
+        a = INV ? make_double2(a.x - b.y, a.y + b.x) : make_double2(a.x + b.y, a.y - b.x);
+    } else {
+        constexpr double c = cos32(NUM);
+        constexpr double t = (INV ? sin32(NUM) : -sin32(NUM)) / cos32(NUM);
+        const double u = fma(-t, b.y, b.x);
+        const double v = fma(t, b.x, b.y);
+        a = make_double2(fma(c, u, a.x), fma(c, v, a.y));
     }
 }
+template <int N, int J = 0>
+__device__ __forceinline__ void lower_half_stage(cplx *y)
+{
+    if constexpr (J < N / 2) {
+        half_butterfly<J * (32 / N), true>(y[J], y[J + N / 2]);
+        lower_half_stage<N, J + 1>(y);
+    }
+}
+// Inverse DFT of N points of which only the lower half of the outputs is wanted:
+// y[n] = sum_d X[d] exp(+2 pi i n d / N), n < N/2, left in x[0..N/2): the last decimation-in-time stage is halved
 template <int N>
 __device__ __forceinline__ void idft_lower_half(cplx *x)
 {
     static_assert(N >= 2 && N <= 32, "radix");
-    cplx e[N / 2], o[N / 2];
+    cplx y[N];
 #pragma unroll
-    for (int d = 0; d < N / 2; ++d) { e[d] = x[2 * d]; o[d] = x[2 * d + 1]; }
-    dft<N / 2, true>(e);
-    dft<N / 2, true>(o);
-    lower_half_stage<N>(x, e, o);
+    for (int k = 0; k < N; ++k) y[k] = x[bitrev<N>(k)];
+    if constexpr (N >= 4) dit_stages_upto<N, 2, N / 2, true>(y);
+    lower_half_stage<N>(y);
+#pragma unroll
+    for (int k = 0; k < N / 2; ++k) x[k] = y[k];
 }
 
 // ------------------------------------------------------------------ plan
