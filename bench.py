@@ -368,7 +368,8 @@ NCU_TRAFFIC: dict = {          # profiles/r1_06_end_of_round.md
     (5, 2): 33.6e6 + 0.4e6,    # rows_inv_kernel<2048>
 }
 # FP64 thread instructions (DADD + DMUL + DFMA) per launch from the same capture; the FP64 pipe issues
-# 64 per clock per SM (ncu sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained)
+# 64 per clock per SM (ncu sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained);
+# the commit after the capture removed about 2 % of cols_kernel's
 NCU_FP64_INSTR: dict = {(5, 0): 0.93e8, (5, 1): 3.51e8, (5, 2): 0.93e8}
 FP64_LANES_PER_CLK_PER_SM = 64
 
