@@ -22,7 +22,10 @@
  * host memory (Fig. 4 :202).
  *
  * Conventions for every call
- *   - Arrays are C order [batch][n_r][n_phi], phi fastest, contiguous, IEEE fp64.
+ *   - Arrays are C order [batch][n_r][n_phi], phi fastest, contiguous, IEEE fp64.  PG_MEM_DEVICE arrays must
+ *     be 16-byte aligned (the kernels move them as 16-byte vectors); a misaligned device pointer is rejected
+ *     with PG_ERR_INVALID_ARG.  Host arrays need 8-byte alignment only.
+ *   - A call leaves the caller's current CUDA device as it found it.
  *   - No C++ types, no exceptions, never abort(): every call returns a pg_status;
  *     pg_last_error() gives the text of the last failure on that solver.
  *   - There is NO CPU fallback and no alternative backend: without a CUDA device of
@@ -82,8 +85,8 @@ pg_status pg_create_ex(pg_solver **out, int n_r, int n_phi, double r_in, double 
 
 /*
  * pg_set_density -- hand the surface density Sigma[batch][n_r][n_phi] to the solver.
- *   PG_MEM_DEVICE      : BORROWED, no copy.  Must stay valid and unmodified until the work of the
- *                        following pg_potential* call has completed on the stream.
+ *   PG_MEM_DEVICE      : BORROWED, no copy, 16-byte aligned.  Must stay valid and unmodified until the work of
+ *                        the following pg_potential* call has completed on the stream.
  *   PG_MEM_HOST_PINNED : cudaMemcpyAsync to an owned device buffer; returns after enqueue; the
  *                        caller must not modify `sigma` until the stream has passed the copy.
  *   PG_MEM_HOST        : memcpy into the owned pinned staging buffer, then cudaMemcpyAsync; returns
@@ -98,7 +101,8 @@ pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspa
  *   PG_MEM_DEVICE / PG_MEM_HOST_PINNED : returns after enqueue (use pg_synchronize or sync the stream).
  *   PG_MEM_HOST                        : blocks until `phi` is filled.
  * For host memspaces with batch > 1 the copies of one field overlap the solves of its neighbours
- * (separate copy stream + events).  `phi` may not alias the density.
+ * (separate copy stream + events).  `phi` may not overlap the density: a PG_MEM_DEVICE `phi` that overlaps a
+ * PG_MEM_DEVICE density is rejected with PG_ERR_INVALID_ARG (no in-place solves).
  */
 pg_status pg_potential(pg_solver *s, double *phi, int batch, pg_memspace where);
 
@@ -130,8 +134,9 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
  *       time pg_potential is called: it is not being written by work still in flight on the stream (it was
  *       produced before a synchronisation, or on another stream that has been joined).  The first forward
  *       kernel may then fetch it while the previous kernel of the stream is still draining (programmatic
- *       dependent launch; the library itself checks that it does not alias the potential its own previous
- *       solve is still writing), and, working alternately in two copies of its intermediate spectrum
+ *       dependent launch; the library itself checks that it does not alias the potential that the
+ *       previous solve ON THE SAME STREAM -- of this or of any other solver of the process -- is still writing; the
+ *       record is kept per stream, so solves on other streams in between do not erase it), and, working alternately in two copies of its intermediate spectrum
  *       (a second workspace of max_batch * (n_phi/2 + 1) * n_r * 16 bytes is allocated on first use), runs
  *       entirely alongside the tail of the previous solve's last kernel.  Time series and batches with
  *       densities resident in HBM (the case bench.py times) qualify; a density written by the caller's

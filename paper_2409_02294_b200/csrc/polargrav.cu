@@ -9,6 +9,7 @@
 
 #include <cmath>
 #include <cstdarg>
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -177,24 +178,61 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 }
 
 // Output range of the last kernel of this library that releases its dependents before it has
-// finished writing (rows_inv_kernel), per process: a rows_fwd_kernel launched right behind it may
-// read its input ahead of griddepcontrol.wait only if that input does not overlap this range.
-// (Any other producer of Sigma on the stream -- a copy, a kernel of the caller -- does not release
-// dependents early, so the launch itself is ordered behind its completion.)
+// finished writing (rows_inv_kernel), PER STREAM: a rows_fwd_kernel launched right behind it on the same
+// stream may read its input ahead of griddepcontrol.wait only if that input does not overlap this range.
+// The programmatic dependency exists only between consecutive kernels of one stream, so the record is keyed
+// by (device, stream): solves of other solvers on other streams in between do not erase it, and two solvers
+// that share a stream see each other's outputs.  (Any other producer of Sigma on the stream -- a copy, a
+// kernel of the caller -- does not release dependents early, so the launch itself is ordered behind its
+// completion; a producer on ANOTHER stream is the caller's promise, PG_OPT_DENSITY_STABLE.)
+struct OutRange { int device; cudaStream_t stream; const char *begin, *end; };
 std::mutex g_out_mutex;
-const char *g_out_begin = nullptr, *g_out_end = nullptr;
+std::vector<OutRange> g_out_ranges;
 
-void note_early_release_output(const void *p, size_t bytes)
+void note_early_release_output(int device, cudaStream_t st, const void *p, size_t bytes)
 {
     std::lock_guard<std::mutex> lock(g_out_mutex);
-    g_out_begin = (const char *)p;
-    g_out_end = g_out_begin + bytes;
+    for (auto &r : g_out_ranges)
+        if (r.device == device && r.stream == st) { r.begin = (const char *)p; r.end = r.begin + bytes; return; }
+    g_out_ranges.push_back(OutRange{device, st, (const char *)p, (const char *)p + bytes});
 }
-bool overlaps_early_release_output(const void *p, size_t bytes)
+bool overlaps_early_release_output(int device, cudaStream_t st, const void *p, size_t bytes)
 {
     std::lock_guard<std::mutex> lock(g_out_mutex);
     const char *b = (const char *)p, *e = b + bytes;
-    return g_out_begin != nullptr && b < g_out_end && g_out_begin < e;
+    for (const auto &r : g_out_ranges)
+        if (r.device == device && r.stream == st) return b < r.end && r.begin < e;
+    return false;
+}
+// a stream that has been synchronised (or is being abandoned) has nothing in flight
+void forget_early_release_output(int device, cudaStream_t st)
+{
+    std::lock_guard<std::mutex> lock(g_out_mutex);
+    for (size_t k = 0; k < g_out_ranges.size(); ++k)
+        if (g_out_ranges[k].device == device && g_out_ranges[k].stream == st) {
+            g_out_ranges[k] = g_out_ranges.back();
+            g_out_ranges.pop_back();
+            return;
+        }
+}
+
+// restores the caller's current device when an ABI call returns
+struct DeviceGuard {
+    int prev = -1;
+    bool changed = false;
+    explicit DeviceGuard(int device)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != device) changed = cudaSetDevice(device) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (changed) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
+
+bool ranges_overlap(const void *a, size_t na, const void *b, size_t nb)
+{
+    const char *a0 = (const char *)a, *b0 = (const char *)b;
+    return a0 < b0 + nb && b0 < a0 + na;
 }
 
 template <int NPHI>
@@ -220,7 +258,7 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
     PG_CUDA(s, launch_pdl(pgk::rows_inv_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, Z, phi, s->d_tw_row,
                           s->d_rs_out, s->n_r, n_items, z_stride, phi_stride));
-    note_early_release_output(phi, (size_t)s->n_r * NPHI * sizeof(double) * batch);
+    note_early_release_output(s->device, st, phi, (size_t)s->n_r * NPHI * sizeof(double) * batch);
     s->launches++;
     return PG_OK;
 }
@@ -424,7 +462,7 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
     // works in the W buffer the previous solve did not use, it depends on nothing in flight (2).
     int early = 0;
     if (s->density_stable && !s->sigma_from_host &&
-        !overlaps_early_release_output(d_sigma, (size_t)batch * s->field * sizeof(double))) {
+        !overlaps_early_release_output(s->device, s->stream, d_sigma, (size_t)batch * s->field * sizeof(double))) {
         early = 1;
         if (d_W == s->d_W && !ev) {
             if (!s->d_W_alt) {
@@ -523,7 +561,7 @@ pg_status create_impl(pg_solver *s)
     PG_CUDA(s, cudaGetDeviceCount(&ndev));
     if (s->device < 0) PG_CUDA(s, cudaGetDevice(&s->device));
     if (s->device >= ndev) { set_err(s, "device %d out of range (%d devices)", s->device, ndev); return PG_ERR_INVALID_ARG; }
-    PG_CUDA(s, cudaSetDevice(s->device));
+    DeviceGuard guard(s->device);      // the caller's current device is restored on return
     cudaDeviceProp prop;
     PG_CUDA(s, cudaGetDeviceProperties(&prop, s->device));
     s->sm_count = prop.multiProcessorCount;
@@ -557,8 +595,8 @@ pg_status create_impl(pg_solver *s)
             s2[j] = (double)(sn * sn);
         }
     }
-    // FFT tables: base roots of the packed row transform (length n_phi/2) and of the n_r-point
-    // column transforms (even and odd-frequency variants), in the layout Plan<L,KIND>::TW_* expects
+    // FFT tables: base roots of the packed row transform (length n_phi/2) and of the zero-padded 2 n_r-point
+    // column transform, in the layout Plan<L,KIND>::TW_* expects
     std::vector<cplx> tw_row, tw_col;
     if (!twiddles_for<pgk::ROW>(s->half, tw_row) || !twiddles_for<pgk::COL>(2 * n_r, tw_col)) {
         set_err(s, "unsupported transform length");
@@ -644,8 +682,9 @@ pg_status pg_create(pg_solver **out, int n_r, int n_phi, double r_in, double r_o
 pg_status pg_destroy(pg_solver *s)
 {
     if (!s) return PG_OK;
-    cudaSetDevice(s->device);
+    DeviceGuard guard(s->device);
     cudaStreamSynchronize(s->stream);
+    forget_early_release_output(s->device, s->stream);
     if (s->h2d) cudaStreamSynchronize(s->h2d);
     if (s->d2h) cudaStreamSynchronize(s->d2h);
     free_all(s);
@@ -659,9 +698,15 @@ pg_status pg_set_density(pg_solver *s, const double *sigma, int batch, pg_memspa
         set_err(s, "pg_set_density: sigma is NULL or batch %d outside [1, %d]", batch, s->max_batch);
         return PG_ERR_INVALID_ARG;
     }
-    PG_CUDA(s, cudaSetDevice(s->device));
+    DeviceGuard guard(s->device);
     const size_t fbytes = s->field * sizeof(double);
     if (where == PG_MEM_DEVICE) {
+        // the kernels move device arrays as 16-byte vectors (cp.async / double2): a misaligned pointer would
+        // raise a sticky "misaligned address" fault that takes the whole CUDA context down
+        if (((uintptr_t)sigma & 15u) != 0) {
+            set_err(s, "pg_set_density: a PG_MEM_DEVICE density must be 16-byte aligned (got %p)", (const void *)sigma);
+            return PG_ERR_INVALID_ARG;
+        }
         s->d_sigma = sigma;
         s->sigma_from_host = false;
     } else if (where == PG_MEM_HOST || where == PG_MEM_HOST_PINNED) {
@@ -708,7 +753,7 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
         set_err(s, "unknown memspace %d", (int)where);
         return PG_ERR_INVALID_ARG;
     }
-    PG_CUDA(s, cudaSetDevice(s->device));
+    DeviceGuard guard(s->device);
     const bool rings = n_rings >= 0;
     if (rings && (ring0 < 0 || n_rings < 1 || ring0 + n_rings > s->n_r)) {
         set_err(s, "ring range [%d, %d) outside [0, %d)", ring0, ring0 + n_rings, s->n_r);
@@ -717,6 +762,19 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
     const size_t out_field = rings ? (size_t)n_rings * s->n_phi : s->field;
     const size_t obytes = out_field * sizeof(double);
     const bool host_out = where != PG_MEM_DEVICE;
+    if (!host_out) {
+        if (((uintptr_t)phi & 15u) != 0) {
+            set_err(s, "a PG_MEM_DEVICE potential must be 16-byte aligned (got %p)", (void *)phi);
+            return PG_ERR_INVALID_ARG;
+        }
+        // `phi` may not alias the density it is computed from (polargrav.h): the last kernel writes Phi rows
+        // while other CTAs of the chain may still be reading Sigma rows of a later field or solve
+        if (!s->sigma_from_host &&
+            ranges_overlap(phi, (size_t)batch * out_field * sizeof(double), s->d_sigma, (size_t)batch * s->field * sizeof(double))) {
+            set_err(s, "phi overlaps the density (in-place solves are not supported)");
+            return PG_ERR_INVALID_ARG;
+        }
+    }
     pg_status st;
     if (host_out) {
         if ((st = ensure_staging(s, false, true)) != PG_OK) return st;
@@ -798,10 +856,11 @@ pg_status pg_grid(const pg_solver *s, double *r, double *phi, double *cell_area)
 pg_status pg_set_stream(pg_solver *s, void *cuda_stream)
 {
     if (!s) return PG_ERR_INVALID_ARG;
-    PG_CUDA(s, cudaSetDevice(s->device));
+    DeviceGuard guard(s->device);
     pg_status st = drain_profile(s);
     if (st != PG_OK) return st;
     PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    forget_early_release_output(s->device, s->stream);
     s->stream = (cudaStream_t)cuda_stream;
     return PG_OK;
 }
@@ -819,10 +878,11 @@ pg_status pg_set_option(pg_solver *s, pg_option option, int value)
 pg_status pg_synchronize(pg_solver *s)
 {
     if (!s) return PG_ERR_INVALID_ARG;
-    PG_CUDA(s, cudaSetDevice(s->device));
+    DeviceGuard guard(s->device);
     PG_CUDA(s, cudaStreamSynchronize(s->h2d));
     PG_CUDA(s, cudaStreamSynchronize(s->stream));
     PG_CUDA(s, cudaStreamSynchronize(s->d2h));
+    forget_early_release_output(s->device, s->stream);
     return PG_OK;
 }
 
@@ -849,6 +909,7 @@ pg_status pg_host_free(void *p)
 pg_status pg_profile(pg_solver *s, int enable)
 {
     if (!s) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
     pg_status st = drain_profile(s);
     if (st != PG_OK) return st;
     s->profile = enable != 0;
@@ -859,6 +920,7 @@ pg_status pg_profile(pg_solver *s, int enable)
 pg_status pg_kernel_times(pg_solver *s, double ms[PG_NUM_KERNELS], long launches[PG_NUM_KERNELS])
 {
     if (!s || !ms || !launches) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
     pg_status st = drain_profile(s);
     if (st != PG_OK) return st;
     for (int k = 0; k < PG_NUM_KERNELS; ++k) { ms[k] = s->prof_ms[k]; launches[k] = s->prof_n[k]; }

@@ -182,3 +182,89 @@ def test_two_solvers_are_independent():
         assert np.abs(pb / oracle.potential_o1(64, 128, 1.0, 50.0, 0.02, sb) - 1).max() <= 1e-9
     finally:
         a.close(); b.close()
+
+
+def test_misaligned_device_pointers_are_rejected(solver):
+    """the kernels move device arrays as 16-byte vectors; a view at an odd element offset must be
+    refused (PG_ERR_INVALID_ARG), not run into a sticky misaligned-address fault."""
+    n = N_R * N_PHI
+    buf = torch.zeros(2 * n + 2, dtype=torch.float64, device="cuda")
+    odd_in, odd_out = buf[1:1 + n], buf[n + 1:2 * n + 1]           # 8 bytes past a 16-byte boundary
+    assert odd_in.data_ptr() % 16 == 8 and odd_out.data_ptr() % 16 == 8
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_set_density(solver.h, odd_in, 1, pg.PG_MEM_DEVICE)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG and "aligned" in pg.last_error(solver.h)
+    sig = torch.from_numpy(random_sigma(N_R, N_PHI, 4)).cuda()
+    pg.pg_set_density(solver.h, sig, 1, pg.PG_MEM_DEVICE)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential(solver.h, odd_out, 1, pg.PG_MEM_DEVICE)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential_direct(solver.h, odd_out, 1, pg.PG_MEM_DEVICE)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    good = torch.empty_like(sig)
+    pg.pg_potential(solver.h, good, 1, pg.PG_MEM_DEVICE)            # the context is still healthy
+    pg.pg_synchronize(solver.h)
+    assert torch.isfinite(good).all()
+
+
+def test_potential_overlapping_the_density_is_rejected(solver):
+    sig = torch.from_numpy(np.stack([random_sigma(N_R, N_PHI, 30 + b) for b in range(2)])).cuda()
+    pg.pg_set_density(solver.h, sig, 2, pg.PG_MEM_DEVICE)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential(solver.h, sig, 2, pg.PG_MEM_DEVICE)          # in place
+    assert e.value.status == pg.PG_ERR_INVALID_ARG and "overlap" in pg.last_error(solver.h)
+    with pytest.raises(pg.PolargravError) as e:
+        pg.pg_potential(solver.h, sig[1:], 2, pg.PG_MEM_DEVICE)      # partial overlap (field 1 onwards)
+    assert e.value.status == pg.PG_ERR_INVALID_ARG
+    out = torch.empty_like(sig)
+    pg.pg_potential(solver.h, out, 2, pg.PG_MEM_DEVICE)
+    pg.pg_synchronize(solver.h)
+    assert (out < 0).all()
+
+
+def test_calls_leave_the_current_device_alone(solver):
+    before = torch.cuda.current_device()
+    sig = random_sigma(N_R, N_PHI, 6)
+    solver.potential_host(sig)
+    pg.pg_synchronize(solver.h)
+    assert torch.cuda.current_device() == before
+
+
+def test_fed_back_potential_with_another_solver_in_between():
+    """the early-fetch alias guard is per stream.  Solver A solves, solver B solves on ANOTHER
+    stream, then A is fed its own (still in flight) potential as the next density with PG_OPT_DENSITY_STABLE on:
+    the library must notice the overlap and fall back to the ordered launch, so the chain equals the same chain
+    run with a synchronisation after every step."""
+    n_r, n_phi = 512, 512
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    A = pg.Solver(n_r, n_phi, 1.0, 1000.0, 0.01, device=0, cuda_stream=sa.cuda_stream)
+    B = pg.Solver(n_r, n_phi, 1.0, 1000.0, 0.01, device=0, cuda_stream=sb.cuda_stream)
+    try:
+        for s in (A, B):
+            pg.pg_set_option(s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        x0 = torch.from_numpy(random_sigma(n_r, n_phi, 77)).cuda()
+        yb = torch.from_numpy(random_sigma(n_r, n_phi, 78)).cuda()
+        torch.cuda.synchronize()
+
+        def chain(sync_every_step):
+            bufs = [x0.clone(), torch.empty_like(x0), torch.empty_like(x0), torch.empty_like(x0)]
+            outb = torch.empty_like(x0)
+            torch.cuda.synchronize()
+            for k in range(3):
+                pg.pg_set_density(A.h, bufs[k], 1, pg.PG_MEM_DEVICE)
+                pg.pg_potential(A.h, bufs[k + 1], 1, pg.PG_MEM_DEVICE)      # A: Phi_k -> next density
+                if sync_every_step:
+                    torch.cuda.synchronize()
+                pg.pg_set_density(B.h, yb, 1, pg.PG_MEM_DEVICE)              # B on another stream in between
+                pg.pg_potential(B.h, outb, 1, pg.PG_MEM_DEVICE)
+                if sync_every_step:
+                    torch.cuda.synchronize()
+            torch.cuda.synchronize()
+            return bufs[3].cpu().numpy()
+
+        ref = chain(True)
+        for _ in range(5):
+            assert np.array_equal(chain(False), ref)
+    finally:
+        A.close(); B.close()

@@ -144,6 +144,94 @@ def test_config4_batch_of_8_vs_oracle():
         d.close()
 
 
+# ---------------------------------------------------------------- whole grids at the bench sizes
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_fft_path_vs_direct_kernel_whole_grid(cfg):
+    """FFT path (a2-a4) against the direct kernel (a5, from coordinates) on EVERY cell of configs 3, 4 (all eight
+    fields) and 5.  a5 itself is tied to the oracle below and in the sampled-ring tests."""
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, _ = d.s.grid()
+        sig = make_batch(cfg, r, phi) if c.batch > 1 else make_sigma(cfg, r, phi)
+        got = d.solve(sig)
+        ref = d.solve(sig, direct=True)
+        if c.batch == 1:
+            assert_parity(got, ref, f"config {cfg} FFT vs direct, whole grid")
+        else:
+            for b in range(c.batch):
+                assert_parity(got[b], ref[b], f"config {cfg} field {b} FFT vs direct, whole grid")
+    finally:
+        d.close()
+
+
+def sample_targets(n_r, n_phi, n, seed):
+    rng = np.random.default_rng(seed)
+    rings = np.concatenate([[0, 0, n_r - 1, n_r - 1, n_r // 2], rng.integers(0, n_r, n - 5)])
+    cols = rng.integers(0, n_phi, n)
+    return (rings.astype(np.int64) * n_phi + cols).astype(np.int64)
+
+
+def test_direct_kernel_vs_definition_oracle_o0():
+    """a5 against O0 -- the four-loop definition from coordinates, NOT the ring-pair oracle O1 whose algorithm
+    direct_tiled_kernel mirrors: every cell of config 1, 320 sampled targets of config 5."""
+    c, d = cfg_solver(1)
+    try:
+        r, phi, _ = d.s.grid()
+        sigma = make_sigma(1, r, phi)
+        ref = oracle.potential_o0(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma)
+        assert_parity(d.solve(sigma, direct=True), ref, "config 1 direct kernel vs O0")
+    finally:
+        d.close()
+    c, d = cfg_solver(5)
+    try:
+        r, phi, _ = d.s.grid()
+        sigma = make_sigma(5, r, phi)
+        tg = sample_targets(c.n_r, c.n_phi, 320, 55)
+        ref = oracle.potential_o0_targets(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, tg)
+        rings = np.unique(tg // c.n_phi)
+        got = {int(i): d.direct_rings(sigma, int(i), 1)[0] for i in rings}
+        got_t = np.array([got[int(t // c.n_phi)][int(t % c.n_phi)] for t in tg])
+        assert_parity(got_t, ref, "config 5 direct kernel vs O0 on sampled targets")
+        fft = d.solve(sigma).reshape(-1)[tg]
+        assert_parity(fft, ref, "config 5 FFT path vs O0 on sampled targets")
+    finally:
+        d.close()
+
+
+def _cached_full_o1(cfg, b, c, sigma):
+    """Full-grid O1 of one field, computed once per box and kept in an untracked cache (minutes of CPU)."""
+    import hashlib, os, tempfile
+    key = hashlib.sha1(sigma.tobytes()).hexdigest()[:16]
+    d = os.path.join(tempfile.gettempdir(), "polargrav_oracle_cache")
+    os.makedirs(d, exist_ok=True)
+    path = os.path.join(d, f"o1_cfg{cfg}_f{b}_{key}.npy")
+    if os.path.exists(path):
+        return np.load(path)
+    ref = oracle.potential_o1(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma)
+    np.save(path, ref)
+    return ref
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_fft_path_vs_full_grid_oracle_at_bench_sizes(cfg):
+    """the parity reference for configs 4-5 is the full-grid O1 result.  Config 5 field 0 (about
+    150 s on 16 host threads) and two fields of config 4 (about 10 s each), element by element."""
+    c, d = cfg_solver(cfg)
+    try:
+        r, phi, _ = d.s.grid()
+        if cfg == 5:
+            sigma = make_sigma(5, r, phi)
+            assert_parity(d.solve(sigma), _cached_full_o1(5, 0, c, sigma), "config 5 whole grid vs O1")
+        else:
+            sig = make_batch(4, r, phi)
+            got = d.solve(sig)
+            for b in (0, 7):
+                assert_parity(got[b], _cached_full_o1(4, b, c, sig[b]), f"config 4 field {b} whole grid vs O1")
+    finally:
+        d.close()
+
+
 # ---------------------------------------------------------------- P4 on the GPU: single cell, no wrap-around
 @pytest.mark.parametrize("n", [64, 256, 2048])
 def test_single_cell_response_no_radial_wraparound(n):
