@@ -98,8 +98,76 @@ class ClockSampler:
 
 dist_env = replicas.dist_env
 
+REL_L2, MAX_REL = 1e-10, 1e-9           # north_star's parity bar (same figures as tests/test_gpu_parity.py)
+REPEATS = 5                              # the K-step region is timed this many times; the median is reported
+
+
+def device_code_hash() -> str:
+    """sha256 over the device code of the library (csrc/fft.cuh + csrc/kernels.cuh): an ncu record applies to
+    the build being timed only if it was captured from the same kernels."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("fft.cuh", "kernels.cuh"):
+        with open(os.path.join(ROOT, "paper_2409_02294_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_record(cfg: int):
+    """profiles/ncu_head.json: DRAM traffic and FP64 instruction counts per launch from the committed
+    `ncu --set full` capture, with the commit and device-code hash it was taken at.  Returned only when that
+    hash equals the hash of the sources this run was built from; otherwise the JSON line carries null and says why."""
+    path = os.path.join(ROOT, "profiles", "ncu_head.json")
+    if not os.path.exists(path):
+        return None, "profiles/ncu_head.json not found"
+    with open(path) as f:
+        rec = json.load(f)
+    if rec.get("device_code_sha256_16") != device_code_hash():
+        return None, (f"profiles/ncu_head.json was captured at commit {rec.get('commit')} from other kernels "
+                      f"(hash {rec.get('device_code_sha256_16')} != {device_code_hash()}): not reported")
+    per_cfg = rec.get("configs", {}).get(str(cfg))
+    if per_cfg is None:
+        return None, f"profiles/ncu_head.json has no capture of config {cfg}"
+    return {"commit": rec.get("commit"), "command": rec.get("command"), **per_cfg}, None
+
+
+def host_placement(gpu_index: int) -> dict:
+    """Where the bench process runs relative to the GPU (section 2.3: up to +220 % on the far socket)."""
+    out = {"cpu_affinity": None, "numa_node_of_process": None, "numa_node_of_gpu": None}
+    try:
+        cpus = sorted(os.sched_getaffinity(0))
+        out["cpu_affinity"] = f"{len(cpus)} cpus: {cpus[0]}-{cpus[-1]}" if cpus else None
+        cpu = cpus[0] if cpus else 0
+        for node in sorted(os.listdir("/sys/devices/system/node")):
+            if node.startswith("node") and os.path.exists(f"/sys/devices/system/node/{node}/cpu{cpu}"):
+                out["numa_node_of_process"] = int(node[4:])
+                break
+    except Exception:
+        pass
+    try:
+        bus = subprocess.run(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=pci.bus_id", "--format=csv,noheader"],
+                             capture_output=True, text=True, timeout=10).stdout.strip().lower()
+        if bus:
+            bus = bus[-12:] if len(bus) > 12 else bus            # 00000000:1B:00.0 -> 0000:1b:00.0
+            with open(f"/sys/bus/pci/devices/{bus}/numa_node") as f:
+                out["numa_node_of_gpu"] = int(f.read().strip())
+    except Exception:
+        pass
+    return out
+
 
 # ------------------------------------------------------------------ CPU oracle legs
+def oracle_rings(cfg: int, n: int):
+    """O1 on n seeded target rings of field 0 of config `cfg` (the parity gate of the bench line)."""
+    import oracle
+    c = CONFIGS[cfg]
+    r, phi, _, _ = oracle.grid(c.n_r, c.n_phi, c.r_in, c.r_out)
+    sigma = make_sigma(cfg, r, phi)
+    rng = np.random.default_rng(1)
+    rings = np.unique(np.concatenate([[0, c.n_r // 2, c.n_r - 1], rng.choice(c.n_r, size=min(c.n_r, n), replace=False)])).astype(np.int32)
+    return rings, oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
+
+
 def oracle_sample(cfg: int, seconds_target: float = 12.0):
     """Times oracle.potential_o1_rings on a bounded sample of target rings of config `cfg`.
     Returns (solves/s extrapolated to the whole grid, cores, description, seconds)."""
@@ -116,13 +184,13 @@ def oracle_sample(cfg: int, seconds_target: float = 12.0):
     waves = int(max(1, min(c.n_r // max(1, len(probe)), round(seconds_target / max(t_probe, 1e-3)))))
     rings = np.sort(rng.choice(c.n_r, size=min(c.n_r, waves * len(probe)), replace=False)).astype(np.int32)
     t0 = time.perf_counter()
-    oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
+    ref = oracle.potential_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, sigma, rings)
     t = time.perf_counter() - t0
     frac = len(rings) / c.n_r
     solves_per_s = frac / t
     desc = (f"oracle O1 (ring-pair direct sum, gcc -O3 -march=native -fopenmp) on {len(rings)} of {c.n_r} "
             f"target rings of config {cfg} field 0 ({t:.2f} s), extrapolated to the whole grid by rings")
-    return solves_per_s, cores, desc, t, rings, sigma
+    return solves_per_s, cores, desc, t, rings, sigma, ref
 
 
 def run_reference(args):
@@ -132,7 +200,7 @@ def run_reference(args):
     import oracle
     cfg = args.config
     c = CONFIGS[cfg]
-    sps, cores, desc, t_one, rings, sigma = oracle_sample(cfg, seconds_target=6.0)
+    sps, cores, desc, t_one, rings, sigma, _ = oracle_sample(cfg, seconds_target=6.0)
     for _ in range(args.warmup):
         pass  # the sample above already warmed caches/threads; the oracle has no other state
     times = []
@@ -157,10 +225,10 @@ def run_reference(args):
     return 0
 
 
-def fp64_block(cfg, dom, ms_per_launch, clocks):
+def fp64_block(n, ms_per_launch, clocks):
     """Secondary roofline of the dominant kernel: FP64 thread instructions per second against the
-    pipe's issue peak 64 x SMs x SM clock (what actually bounds cols_kernel)."""
-    n = NCU_FP64_INSTR.get((cfg, dom))
+    pipe's issue peak 64 x SMs x SM clock (what actually bounds cols_kernel).
+    n = FP64 thread instructions per launch from profiles/ncu_head.json (None when no valid record)."""
     if n is None or ms_per_launch <= 0:
         return None
     import torch
@@ -231,17 +299,23 @@ def run_ours(args):
     pg.pg_synchronize(h)
 
     # ---- timed region: exactly K steps between CUDA events on the solver's stream
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # The region of exactly K steps is timed REPEATS times (barrier + synchronize on both sides of each); the
+    # median of the repeats is the reported figure, min and max go beside it (median of 5).
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    barrier(); torch.cuda.synchronize()
+    rep_ms = []
     n0 = pg.pg_launch_count(h)
-    e0.record(st)
-    for k in range(args.steps):
-        step(k)
-    e1.record(st)
-    torch.cuda.synchronize(); barrier()
+    for _ in range(REPEATS):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier(); torch.cuda.synchronize()
+        e0.record(st)
+        for k in range(args.steps):
+            step(k)
+        e1.record(st)
+        torch.cuda.synchronize(); barrier()
+        rep_ms.append(max_over_ranks(e0.elapsed_time(e1)))
     n1 = pg.pg_launch_count(h)
-    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    ms_total = float(np.median(rep_ms))
+    gate_field = d_phi[0][0].cpu().numpy() if rank == 0 else None     # field 0 as the timed region left it
     # keep the GPU busy a little longer so that short runs still collect clock samples under load
     if sampler is not None:
         t_end = time.perf_counter() + 0.6
@@ -252,8 +326,21 @@ def run_ours(args):
                 pg.pg_synchronize(h)
         pg.pg_synchronize(h)
     clocks = sampler.stop() if sampler is not None else None
+    # ---- parity gate ("parity gate before any timing counts"): the potential of field 0 as the timed
+    # loop left it in HBM, against oracle O1 on seeded rings.  Steps k = 0 (mod R) solve field 0 into d_phi[0].
+    parity = {"ok": True, "what": "rank 0 only"}
+    if rank == 0:
+        gate_rings, gate_ref = oracle_rings(cfg, 12 if c.n_r >= 1024 else 32)
+        gate_got = gate_field[gate_rings]
+        gate_l2 = float(np.linalg.norm(gate_got - gate_ref) / np.linalg.norm(gate_ref))
+        gate_mx = float(np.abs(gate_got / gate_ref - 1.0).max())
+        parity = {"rel_l2": gate_l2, "max_rel": gate_mx, "rings": int(len(gate_rings)),
+                  "bar": {"rel_l2": REL_L2, "max_rel": MAX_REL},
+                  "what": "d_phi of field 0 as the timed region left it vs oracle O1 (ring-pair direct sum) on seeded rings",
+                  "ok": bool(gate_l2 <= REL_L2 and gate_mx <= MAX_REL)}
     ms_per_step = ms_total / args.steps
     value = world * c.batch * 1e3 / ms_per_step
+    n_launch = int(round((n1 - n0) / REPEATS)) * world
 
     # ---- per-kernel durations (events around every kernel, separate pass) -> roofline of the dominant kernel
     pg.pg_profile(h, True)
@@ -264,6 +351,7 @@ def run_ours(args):
     per_launch_ms = [kms[i] / max(1, kn[i]) for i in range(pg.PG_NUM_KERNELS)]
     dom = int(np.argmax(per_launch_ms))
     peak, peak_src = load_peaks()
+    ncu, ncu_why = ncu_record(cfg)
     kbytes = [pg.pg_kernel_algorithmic_bytes(h, i, c.batch) for i in range(pg.PG_NUM_KERNELS)]
     achieved = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
     path_bytes = pg.pg_algorithmic_bytes(h, c.batch)
@@ -325,17 +413,23 @@ def run_ours(args):
                    "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
                          f"{R * pair_bytes / 1e6:.0f} MB in total vs 126 MB L2"},
         "cells_per_s": value * c.n_r * c.n_phi,
-        "gpu_launches": int((n1 - n0) * world),
+        "gpu_launches": n_launch,
+        "repeats": {"n": REPEATS, "ms_per_step_median": ms_per_step, "ms_per_step_min": min(rep_ms) / args.steps,
+                    "ms_per_step_max": max(rep_ms) / args.steps},
+        "parity": parity,
+        "host": host_placement(local_rank),
         "roofline": {
             "bound": "hbm", "kernel": pg.KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg, dom)), "peak_source": peak_src,
+            "frac": achieved / peak, "traffic": (ncu or {}).get("dram_bytes_per_launch", [None] * 3)[dom],
+            "traffic_source": (f"profiles/ncu_head.json, ncu --set full at commit {ncu['commit']}" if ncu else ncu_why),
+            "peak_source": peak_src,
             "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
             "kernels": {pg.KERNEL_NAMES[i]: {"ms": per_launch_ms[i], "alg_bytes": kbytes[i],
                                             "gbs": kbytes[i] / (per_launch_ms[i] * 1e-3) / 1e9 if per_launch_ms[i] > 0 else None}
                         for i in range(pg.PG_NUM_KERNELS)},
             "path": {"alg_bytes_per_step": path_bytes, "gbs": path_gbs, "frac_of_peak": path_gbs / peak,
                      "frac_of_8TBs_nominal": path_gbs / 8000.0},
-            "fp64": fp64_block(cfg, dom, per_launch_ms[dom], clocks),
+            "fp64": fp64_block((ncu or {}).get("fp64_thread_instructions_per_launch", [None] * 3)[dom], per_launch_ms[dom], clocks),
             "l2_flushed_ms_per_step": ms_flushed, "l2_flushed_frac_of_peak": path_bytes / (ms_flushed * 1e-3) / 1e9 / peak,
         },
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * c.batch,
@@ -346,7 +440,7 @@ def run_ours(args):
         "clocks": clocks,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        sps, cores, desc, _, _, _ = oracle_sample(cfg)
+        sps, cores, desc, _, _, _, _ = oracle_sample(cfg)
         line["cpu_baseline"] = {"value": sps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
     for a in pin_in + pin_out:
         a.free()
@@ -357,20 +451,12 @@ def run_ours(args):
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+    if not parity["ok"]:
+        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {parity}; the timing above does not count\n")
+        return 3
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/), keyed by (config, kernel index).  Filled in from profiles/*.md; None = not captured.
-NCU_TRAFFIC: dict = {          # profiles/r1_06_end_of_round.md
-    (5, 0): 33.6e6 + 0.9e6,    # rows_fwd_kernel<2048>
-    (5, 1): 67.2e6 + 1.0e6,    # cols_kernel<2048>
-    (5, 2): 33.6e6 + 0.4e6,    # rows_inv_kernel<2048>
-}
-# FP64 thread instructions (DADD + DMUL + DFMA) per launch from the same capture; the FP64 pipe issues
-# 64 per clock per SM (ncu sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained);
-# the commit after the capture removed about 2 % of cols_kernel's
-NCU_FP64_INSTR: dict = {(5, 0): 0.93e8, (5, 1): 3.51e8, (5, 2): 0.93e8}
 FP64_LANES_PER_CLK_PER_SM = 64
 
 
@@ -417,6 +503,108 @@ def run_direct(args):
     return 0
 
 
+def run_staging(args):
+    """--staging: row a6's own measurement.  The paper times the host-to-device
+    transfer of one 128^3 array: about 1 ms from pinned memory, about 3 ms from pageable memory (A100 40 GB, PCIe).
+    Here the same 16.8 MB (128^3 fp64 = a 1024 x 2048 grid) goes through the library's own staging calls,
+    PG_MEM_HOST (pageable: memcpy into the owned pinned buffer, then cudaMemcpyAsync) against PG_MEM_HOST_PINNED
+    (cudaMemcpyAsync straight from the caller's pinned buffer), upload and download separately; then the batch
+    pipeline of config 4 (8 fields): upload-only, solve-only, download-only and all three overlapped."""
+    import torch
+    from paper_2409_02294_b200 import binding as pg, build as pg_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    reps = max(5, min(args.steps, 30))
+
+    def med(f, n=reps):
+        ts = []
+        for _ in range(n):
+            t0 = time.perf_counter(); f(); ts.append(time.perf_counter() - t0)
+        return 1e3 * float(np.median(ts))
+
+    st = torch.cuda.Stream()
+    n_r, n_phi = 1024, 2048                                  # 2^21 cells = 128^3
+    s = pg.Solver(n_r, n_phi, 1.0, 1000.0, 0.01, device=0, cuda_stream=st.cuda_stream)
+    h = s.h
+    from paper_2409_02294_b200.workloads import random_sigma
+    sig = random_sigma(n_r, n_phi, 1)
+    pin_in, pin_out = pg.PinnedArray((n_r, n_phi)), pg.PinnedArray((n_r, n_phi))
+    pin_in.array[...] = sig
+    page_in, page_out = sig.copy(), np.empty_like(sig)
+    d_sig = torch.from_numpy(sig).cuda(); d_phi = torch.empty_like(d_sig)
+    nbytes = sig.nbytes
+
+    def up(mem, buf):
+        pg.pg_set_density(h, buf, 1, mem); pg.pg_synchronize(h)
+
+    def solve_dev():
+        pg.pg_set_density(h, d_sig, 1, pg.PG_MEM_DEVICE); pg.pg_potential(h, d_phi, 1, pg.PG_MEM_DEVICE); pg.pg_synchronize(h)
+
+    def solve_to(mem, buf):
+        pg.pg_set_density(h, d_sig, 1, pg.PG_MEM_DEVICE); pg.pg_potential(h, buf, 1, mem); pg.pg_synchronize(h)
+
+    for _ in range(3):
+        up(pg.PG_MEM_HOST_PINNED, pin_in.ptr); up(pg.PG_MEM_HOST, page_in); solve_dev()
+        solve_to(pg.PG_MEM_HOST_PINNED, pin_out.ptr); solve_to(pg.PG_MEM_HOST, page_out)
+    h2d_pinned = med(lambda: up(pg.PG_MEM_HOST_PINNED, pin_in.ptr))
+    h2d_pageable = med(lambda: up(pg.PG_MEM_HOST, page_in))
+    t_solve = med(solve_dev)
+    d2h_pinned = med(lambda: solve_to(pg.PG_MEM_HOST_PINNED, pin_out.ptr)) - t_solve
+    d2h_pageable = med(lambda: solve_to(pg.PG_MEM_HOST, page_out)) - t_solve
+    ok = bool(np.array_equal(pin_out.array, page_out) and (page_out < 0).all())
+    pin_in.free(); pin_out.free(); s.close()
+
+    # ---- the batch pipeline of config 4: H2D(b+1) || solve(b) || D2H(b-1)
+    c = CONFIGS[4]
+    s = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, max_batch=c.batch, device=0, cuda_stream=st.cuda_stream)
+    h = s.h
+    shape = (c.batch, c.n_r, c.n_phi)
+    pin_in, pin_out = pg.PinnedArray(shape), pg.PinnedArray(shape)
+    r, phi, _ = s.grid()
+    pin_in.array[...] = np.stack([make_sigma(4, r, phi, b) for b in range(c.batch)])
+    d_b = torch.from_numpy(pin_in.array.copy()).cuda(); d_o = torch.empty_like(d_b)
+
+    def b_up():
+        pg.pg_set_density(h, pin_in.ptr, c.batch, pg.PG_MEM_HOST_PINNED); pg.pg_synchronize(h)
+
+    def b_solve():
+        pg.pg_set_density(h, d_b, c.batch, pg.PG_MEM_DEVICE); pg.pg_potential(h, d_o, c.batch, pg.PG_MEM_DEVICE); pg.pg_synchronize(h)
+
+    def b_down():
+        pg.pg_set_density(h, d_b, c.batch, pg.PG_MEM_DEVICE); pg.pg_potential(h, pin_out.ptr, c.batch, pg.PG_MEM_HOST_PINNED); pg.pg_synchronize(h)
+
+    def b_all(n=6):
+        for _ in range(n):
+            pg.pg_set_density(h, pin_in.ptr, c.batch, pg.PG_MEM_HOST_PINNED)
+            pg.pg_potential(h, pin_out.ptr, c.batch, pg.PG_MEM_HOST_PINNED)
+        pg.pg_synchronize(h)
+
+    for _ in range(2):
+        b_up(); b_solve(); b_down(); b_all(2)
+    t_up, t_sv = med(b_up, 10), med(b_solve, 10)
+    t_dn = med(b_down, 10) - t_sv
+    t_all = med(b_all, 5) / 6
+    pin_in.free(); pin_out.free(); s.close()
+    gbs = lambda ms: nbytes / (ms * 1e-3) / 1e9
+    line = {
+        "metric": "host staging of one 128^3 fp64 array (16.8 MB) through pg_set_density / pg_potential (row a6)",
+        "unit": "ms", "n_gpus": 1, "dtype": "f64", "data": "synthetic", "repeats": reps,
+        "h2d": {"pinned_ms": h2d_pinned, "pageable_ms": h2d_pageable, "pinned_gbs": gbs(h2d_pinned), "pageable_gbs": gbs(h2d_pageable)},
+        "d2h": {"pinned_ms": d2h_pinned, "pageable_ms": d2h_pageable, "pinned_gbs": gbs(d2h_pinned), "pageable_gbs": gbs(d2h_pageable),
+                "how": "pg_potential into a host buffer minus the device-resident solve of the same grid"},
+        "solve_ms_1024x2048": t_solve, "outputs_equal_and_sane": ok,
+        "paper": {"h2d_pinned_ms": 1.0, "h2d_pageable_ms": 3.0, "hardware": "A100 40 GB, PCIe host link", "source": "PAPER.md:119 (section 2.2.2)"},
+        "pipeline_config4": {"batch": c.batch, "bytes_each_way": int(np.prod(shape)) * 8, "upload_only_ms": t_up, "solve_only_ms": t_sv,
+                             "download_only_ms": t_dn, "sum_ms": t_up + t_sv + t_dn, "pipelined_ms_per_batch": t_all,
+                             "note": "pipelined is close to max(upload, download), not to the sum: H2D(b+1), solve(b) and D2H(b-1) overlap"},
+        "host": host_placement(0),
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -426,9 +614,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
+    ap.add_argument("--staging", action="store_true", help="time row a6 alone: pinned vs pageable staging of a 128^3 array (PAPER.md:119)")
     args = ap.parse_args()
     if args.direct:
         return run_direct(args)
+    if args.staging:
+        return run_staging(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)
