@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "polar_oracle.c")
+_SRC_EXT = os.path.join(_HERE, "polar_oracle_ext.c")      # NEXT-4 variants: softening modes, acceleration
 _LIB = None
 
 
@@ -30,6 +31,8 @@ def _machine_tag() -> str:
         pass
     with open(_SRC, "rb") as f:
         src = f.read()
+    with open(_SRC_EXT, "rb") as f:
+        src += f.read()
     return hashlib.sha1(flags.encode() + src).hexdigest()[:12]
 
 
@@ -43,7 +46,7 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(path):
         tmp = path + f".tmp{os.getpid()}"
         cmd = ["gcc", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared",
-               "-o", tmp, _SRC, "-lm"]
+               "-o", tmp, _SRC, _SRC_EXT, "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, path)
     return path
@@ -61,8 +64,10 @@ def _lib():
         L.po_potential_o0_full.argtypes = [i, i, d, d, d, p, p]
         L.po_potential_o1_rings.argtypes = [i, i, d, d, d, p, p, i, p]
         L.po_potential_o1_full.argtypes = [i, i, d, d, d, p, p]
+        L.po_ext_o0_targets.argtypes = [i, i, d, d, d, i, p, p, l, p, p, p]
+        L.po_ext_o1_rings.argtypes = [i, i, d, d, d, i, p, p, i, p, p, p]
         for fn in (L.po_grid, L.po_potential_o0_targets, L.po_potential_o0_full,
-                   L.po_potential_o1_rings, L.po_potential_o1_full):
+                   L.po_potential_o1_rings, L.po_potential_o1_full, L.po_ext_o0_targets, L.po_ext_o1_rings):
             fn.restype = i
         _LIB = L
     return _LIB
@@ -130,3 +135,39 @@ def potential_o1_rings(n_r, n_phi, r_in, r_out, eps, sigma, rings):
                                         rg.ctypes.data, rg.size, out.ctypes.data),
            "po_potential_o1_rings")
     return out
+
+
+# ------------------------------------------------------------------ NEXT-4 variants (polar_oracle_ext.c)
+SOFT_SYMMETRIC, SOFT_FIELD, SOFT_SOURCE = 0, 1, 2
+
+
+def ext_o0_targets(n_r, n_phi, r_in, r_out, eps, soft, sigma, targets):
+    """Definition (readings N1, N2) at flat target indices. Returns (Phi, a_r, a_phi)."""
+    s = _sigma(sigma, n_r, n_phi)
+    t = np.ascontiguousarray(targets, dtype=np.int64)
+    if t.size and (t.min() < 0 or t.max() >= n_r * n_phi):
+        raise ValueError("target index out of range")
+    out = [np.empty(t.size) for _ in range(3)]
+    _check(_lib().po_ext_o0_targets(n_r, n_phi, r_in, r_out, eps, int(soft), s.ctypes.data, t.ctypes.data, t.size,
+                                    out[0].ctypes.data, out[1].ctypes.data, out[2].ctypes.data), "po_ext_o0_targets")
+    return tuple(out)
+
+
+def ext_o0(n_r, n_phi, r_in, r_out, eps, soft, sigma):
+    """Definition on the whole grid. Returns (Phi, a_r, a_phi), each [n_r][n_phi]."""
+    out = ext_o0_targets(n_r, n_phi, r_in, r_out, eps, soft, sigma, np.arange(n_r * n_phi))
+    return tuple(x.reshape(n_r, n_phi) for x in out)
+
+
+def ext_o1_rings(n_r, n_phi, r_in, r_out, eps, soft, sigma, rings):
+    """Ring-pair form on target rings. Returns (Phi, a_r, a_phi), each [len(rings)][n_phi]."""
+    s = _sigma(sigma, n_r, n_phi)
+    rg = np.ascontiguousarray(rings, dtype=np.int32)
+    out = [np.empty((rg.size, n_phi)) for _ in range(3)]
+    _check(_lib().po_ext_o1_rings(n_r, n_phi, r_in, r_out, eps, int(soft), s.ctypes.data, rg.ctypes.data, rg.size,
+                                  out[0].ctypes.data, out[1].ctypes.data, out[2].ctypes.data), "po_ext_o1_rings")
+    return tuple(out)
+
+
+def ext_o1(n_r, n_phi, r_in, r_out, eps, soft, sigma):
+    return ext_o1_rings(n_r, n_phi, r_in, r_out, eps, soft, sigma, np.arange(n_r))
