@@ -117,6 +117,30 @@ pg_status pg_potential(pg_solver *s, double *phi, int batch, pg_memspace where);
 pg_status pg_potential_direct(pg_solver *s, double *phi, int batch, pg_memspace where);
 pg_status pg_potential_direct_rings(pg_solver *s, double *phi, int ring0, int n_rings, pg_memspace where);
 
+/* ---------------------------------------------------------------- variants of the path
+ * Not in the paper (PAPER.md:267 only names the convolution method); readings N1 and N2 of DESIGN.md section 3.
+ *
+ * pg_set_softening -- which cell lends its size to the softening length of a pair (field ring i, source ring i'):
+ *     PG_SOFT_SYMMETRIC  eps^2 h_i h_i'   (default; the pair kernel is even in the radial lag, its spectrum real)
+ *     PG_SOFT_FIELD      eps^2 h_i^2      (softening length of the field cell)
+ *     PG_SOFT_SOURCE     eps^2 h_i'^2     (softening length of the source cell)
+ * All three depend on index differences only (eps is dimensionless), so the FFT convolution stays exact; for the
+ * last two the kernel spectrum is complex and the column pass multiplies complex by complex.  Blocking: it
+ * synchronises the stream and rebuilds the spectrum.  Affects pg_potential and pg_acceleration; the direct kernel
+ * (pg_potential_direct*) always uses the symmetric form.
+ *
+ * pg_acceleration -- the softened pair acceleration of the density last set, in the polar basis of the field cell,
+ *     a_r   = - sum Sigma' dA' (r - r' cos(phi - phi')) / d2^(3/2),
+ *     a_phi = - sum Sigma' dA'  r' sin(phi - phi')      / d2^(3/2),      d2 as in the header of this file,
+ * with the softening length of each pair held fixed (the force law hydro codes apply; equal to -grad Phi for
+ * PG_SOFT_SOURCE).  Two more convolutions that share the forward transform of the density with each other.
+ * a_r, a_phi: [batch][n_r][n_phi] each, same memspace; they may overlap neither each other nor the density.
+ * PG_MEM_DEVICE returns after enqueue; host memspaces block until both arrays are filled.  The two kernel
+ * spectra are built on the first call (and again after pg_set_softening). */
+typedef enum { PG_SOFT_SYMMETRIC = 0, PG_SOFT_FIELD = 1, PG_SOFT_SOURCE = 2 } pg_softening;
+pg_status pg_set_softening(pg_solver *s, pg_softening mode);
+pg_status pg_acceleration(pg_solver *s, double *a_r, double *a_phi, int batch, pg_memspace where);
+
 /* pg_destroy -- frees everything the solver owns. pg_destroy(NULL) is a no-op returning PG_OK. */
 pg_status pg_destroy(pg_solver *s);
 

@@ -19,6 +19,7 @@ PG_ERR_INVALID_ARG, PG_ERR_UNSUPPORTED, PG_ERR_CUDA, PG_ERR_NOMEM, PG_ERR_STATE 
 PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
 PG_NUM_KERNELS = 3
 PG_OPT_DENSITY_STABLE = 1
+PG_SOFT_SYMMETRIC, PG_SOFT_FIELD, PG_SOFT_SOURCE = 0, 1, 2
 KERNEL_NAMES = ("rows_fwd(a2)", "cols(a3+a4r)", "rows_inv(a4phi)")
 
 # every symbol include/polargrav.h declares
@@ -27,7 +28,7 @@ EXPORTS = (
     "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_set_option", "pg_synchronize",
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
-    "pg_version",
+    "pg_version", "pg_set_softening", "pg_acceleration",
 )
 
 _lib = None
@@ -55,6 +56,8 @@ def lib():
         L.pg_potential.argtypes = [vp, vp, i, i]
         L.pg_potential_direct.argtypes = [vp, vp, i, i]
         L.pg_potential_direct_rings.argtypes = [vp, vp, i, i, i]
+        L.pg_set_softening.argtypes = [vp, i]
+        L.pg_acceleration.argtypes = [vp, vp, vp, i, i]
         L.pg_destroy.argtypes = [vp]
         L.pg_grid.argtypes = [vp, vp, vp, vp]
         L.pg_set_stream.argtypes = [vp, vp]
@@ -136,6 +139,14 @@ def pg_potential_direct(h, phi, batch, where):
 
 def pg_potential_direct_rings(h, phi, ring0, n_rings, where):
     _check(lib().pg_potential_direct_rings(h, _ptr(phi), ring0, n_rings, where), h)
+
+
+def pg_set_softening(h, mode):
+    _check(lib().pg_set_softening(h, int(mode)), h)
+
+
+def pg_acceleration(h, a_r, a_phi, batch, where):
+    _check(lib().pg_acceleration(h, _ptr(a_r), _ptr(a_phi), batch, where), h)
 
 
 def pg_destroy(h):

@@ -6,6 +6,7 @@
 // fallback: without an sm_100 device pg_create* fails.
 #include "../../include/polargrav.h"
 #include "kernels.cuh"
+#include "variants.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -50,6 +51,13 @@ struct pg_solver {
     cplx *d_tw_row = nullptr;     // Plan<n_phi/2, ROW> twiddle table
     cplx *d_tw_col = nullptr;     // Plan<2 n_r, COL> twiddle table
     double *d_rs_in = nullptr, *d_rs_out = nullptr;
+    // NEXT-4 variants (variants.cuh): softening mode, complex kernel spectra [Phi, a_r, a_phi] for it, the post-scale
+    // r^(-3/2) of the acceleration, and a second spectrum workspace (the column pass is out of place there)
+    int soft = PG_SOFT_SYMMETRIC;
+    cplx *d_khat_c[3] = {nullptr, nullptr, nullptr};
+    bool khat_c_valid[3] = {false, false, false};
+    double *d_rs_out32 = nullptr;
+    cplx *d_W_var = nullptr;
     double *d_r = nullptr, *d_dA = nullptr, *d_s2 = nullptr;
     // [max_batch][n_r][n_phi] each, lazily allocated, TWO slots per direction: the upload of the next
     // density does not wait for the solve that still reads the previous one, and a solve does not wait for
@@ -251,13 +259,13 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
 
 template <int NPHI>
 pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, long z_stride, long phi_stride,
-                          cudaStream_t st)
+                          cudaStream_t st, const double *oscale)
 {
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (s->n_r / S::ROWS) * batch;
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
     PG_CUDA(s, launch_pdl(pgk::rows_inv_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, Z, phi, s->d_tw_row,
-                          s->d_rs_out, s->n_r, n_items, z_stride, phi_stride));
+                          oscale, s->n_r, n_items, z_stride, phi_stride));
     note_early_release_output(s->device, st, phi, (size_t)s->n_r * NPHI * sizeof(double) * batch);
     s->launches++;
     return PG_OK;
@@ -282,6 +290,30 @@ pg_status launch_khat_cols(pg_solver *s, const cplx *ZK, double scale, cudaStrea
     const size_t smem = (size_t)pgk::Plan<2 * NR, pgk::COL>::LINE * sizeof(cplx);
     pgk::khat_cols_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, s->d_khat, s->d_tw_col, scale);
     PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+template <int NR>
+pg_status launch_khat_cols_cplx(pg_solver *s, const cplx *ZK, cplx *out, double scale, cudaStream_t st)
+{
+    const int threads = NR / 8;
+    const size_t smem = (size_t)pgk::Plan<2 * NR, pgk::COL>::LINE * sizeof(cplx);
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::khat_cols_cplx_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    pgk::khat_cols_cplx_kernel<NR><<<s->half + 1, threads, smem, st>>>(ZK, out, s->d_tw_col, scale);
+    PG_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+template <int NR>
+pg_status launch_cols_cplx(pg_solver *s, const cplx *src, cplx *dst, const cplx *khat_c, int batch, long z_stride, cudaStream_t st)
+{
+    typedef pgk::ColShape<NR> S;
+    const int modes = s->half + 1;
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::cols_cplx_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::LINES));
+    dim3 grid((modes + S::MODES - 1) / S::MODES, batch);
+    PG_CUDA(s, launch_pdl(pgk::cols_cplx_kernel<NR>, grid, dim3(S::THREADS), S::LINES, st, src, dst, khat_c,
+                          (const cplx *)s->d_tw_col, modes, z_stride));
     s->launches++;
     return PG_OK;
 }
@@ -334,9 +366,10 @@ pg_status rows_fwd(pg_solver *s, const double *sigma, cplx *W, const double *rsc
 #undef CALL
 }
 pg_status rows_inv(pg_solver *s, const cplx *W, double *phi, int batch, long w_stride, long phi_stride,
-                   cudaStream_t st)
+                   cudaStream_t st, const double *oscale = nullptr)
 {
-#define CALL(N) launch_rows_inv<N>(s, W, phi, batch, w_stride, phi_stride, st)
+    if (!oscale) oscale = s->d_rs_out;
+#define CALL(N) launch_rows_inv<N>(s, W, phi, batch, w_stride, phi_stride, st, oscale)
     PG_DISPATCH(s->n_phi, CALL)
 #undef CALL
 }
@@ -355,6 +388,18 @@ pg_status prepare_kernels_rows(pg_solver *s)
 pg_status prepare_kernels_cols(pg_solver *s)
 {
 #define CALL(N) prepare_cols<N>(s)
+    PG_DISPATCH(s->n_r, CALL)
+#undef CALL
+}
+pg_status khat_cols_cplx(pg_solver *s, const cplx *Wk, cplx *out, double scale, cudaStream_t st)
+{
+#define CALL(N) launch_khat_cols_cplx<N>(s, Wk, out, scale, st)
+    PG_DISPATCH(s->n_r, CALL)
+#undef CALL
+}
+pg_status cols_cplx(pg_solver *s, const cplx *src, cplx *dst, const cplx *khat_c, int batch, long w_stride, cudaStream_t st)
+{
+#define CALL(N) launch_cols_cplx<N>(s, src, dst, khat_c, batch, w_stride, st)
     PG_DISPATCH(s->n_r, CALL)
 #undef CALL
 }
@@ -404,6 +449,78 @@ pg_status build_khat(pg_solver *s)
     cudaFree(d_kpad);
     cudaFree(d_wk);
     return st;
+}
+
+// Complex spectrum of one of the variant kernels (variants.cuh: kind 0 = K_Phi, 1 = K_r, 2 = K_phi) for the
+// solver's softening mode; same pipeline and normalisation as build_khat, the column pass keeps the complex value.
+pg_status build_khat_variant(pg_solver *s, int kind)
+{
+    if (s->khat_c_valid[kind]) return PG_OK;
+    const int n_r = s->n_r, n_phi = s->n_phi;
+    const size_t kpad_n = (size_t)2 * n_r * n_phi;
+    const size_t wk_n = (size_t)(s->half + 1) * 2 * n_r;
+    if (!s->d_khat_c[kind]) PG_CUDA(s, cudaMalloc((void **)&s->d_khat_c[kind], wk_n * sizeof(cplx)));
+    if (!s->d_rs_out32) {
+        std::vector<double> w(n_r);
+        for (int i = 0; i < n_r; ++i) w[i] = (double)(1.0L / ((long double)s->r[i] * sqrtl((long double)s->r[i])));
+        pg_status up = upload(s, &s->d_rs_out32, w);
+        if (up != PG_OK) return up;
+    }
+    double *d_kpad = nullptr;
+    cplx *d_wk = nullptr;
+    PG_CUDA(s, cudaMalloc((void **)&d_kpad, kpad_n * sizeof(double)));
+    if (cudaMalloc((void **)&d_wk, wk_n * sizeof(cplx)) != cudaSuccess) {
+        cudaFree(d_kpad);
+        set_err(s, "cudaMalloc(kernel workspace) failed");
+        return PG_ERR_NOMEM;
+    }
+    pg_status st = PG_OK;
+    do {
+        const double eta2 = s->eps * s->eps * std::sinh(s->du) * s->dphi;
+        const int threads = 256;
+        const long blocks = (long)((kpad_n + threads - 1) / threads);
+        pgk::green_fill_var_kernel<<<(unsigned)blocks, threads, 0, s->stream>>>(d_kpad, n_r, n_phi, s->du, eta2, s->soft, kind);
+        s->launches++;
+        if (cudaGetLastError() != cudaSuccess) { st = PG_ERR_CUDA; break; }
+        st = rows_fwd(s, d_kpad, d_wk, nullptr, 2 * n_r, 1, 0, 0, s->stream, 0);
+        if (st != PG_OK) break;
+        const double scale = -std::sinh(s->du) * s->dphi / (8.0 * (double)n_r * (double)n_phi);
+        st = khat_cols_cplx(s, d_wk, s->d_khat_c[kind], scale, s->stream);
+        if (st != PG_OK) break;
+        if (cudaStreamSynchronize(s->stream) != cudaSuccess) { st = PG_ERR_CUDA; break; }
+    } while (0);
+    if (st == PG_ERR_CUDA && s->err[0] == 0) set_err(s, "variant kernel precompute failed: %s", cudaGetErrorString(cudaGetLastError()));
+    cudaFree(d_kpad);
+    cudaFree(d_wk);
+    if (st == PG_OK) s->khat_c_valid[kind] = true;
+    return st;
+}
+
+pg_status ensure_var_workspace(pg_solver *s)
+{
+    if (!s->d_W_var) {
+        const size_t w_bytes = (size_t)s->max_batch * (s->half + 1) * s->n_r * sizeof(cplx);
+        PG_CUDA(s, cudaMalloc((void **)&s->d_W_var, w_bytes));
+    }
+    return PG_OK;
+}
+
+// rows_fwd once, then one (complex column pass, inverse row pass) per requested output
+pg_status solve_variant(pg_solver *s, const double *d_sigma, cplx *d_W, int batch, int n_out, const int *kinds,
+                        double *const *outs)
+{
+    const long fs = (long)s->field, ws = (long)(s->half + 1) * s->n_r;
+    pg_status st = ensure_var_workspace(s);
+    if (st != PG_OK) return st;
+    for (int q = 0; q < n_out; ++q)
+        if ((st = build_khat_variant(s, kinds[q])) != PG_OK) return st;
+    if ((st = rows_fwd(s, d_sigma, d_W, s->d_rs_in, s->n_r, batch, fs, ws, s->stream, 0)) != PG_OK) return st;
+    s->last_w = d_W;
+    for (int q = 0; q < n_out; ++q) {
+        if ((st = cols_cplx(s, d_W, s->d_W_var, s->d_khat_c[kinds[q]], batch, ws, s->stream)) != PG_OK) return st;
+        if ((st = rows_inv(s, s->d_W_var, outs[q], batch, ws, fs, s->stream, kinds[q] == 0 ? s->d_rs_out : s->d_rs_out32)) != PG_OK) return st;
+    }
+    return PG_OK;
 }
 
 pg_status ensure_staging(pg_solver *s, bool need_in, bool need_out)
@@ -456,6 +573,12 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         }
         ev = &s->prof_pool[s->prof_used++];
         PG_CUDA(s, cudaEventRecord(ev->e[0], s->stream));
+    }
+    if (s->soft != PG_SOFT_SYMMETRIC) {
+        // field / source softening: complex spectrum, variants.cuh (no per-kernel profiling on this path)
+        const int kind = 0;
+        double *out = d_phi;
+        return solve_variant(s, d_sigma, d_W, batch, 1, &kind, &out);
     }
     // How much rows_fwd depends on the kernel before it (kernels.cuh): with a stable density that does not
     // alias the potential still being written, the first item is fetched early (1); if the solve also
@@ -535,7 +658,8 @@ void free_all(pg_solver *s)
 {
     if (!s) return;
     cudaFree(s->d_W); cudaFree(s->d_W_alt); cudaFree(s->d_khat); cudaFree(s->d_tw_row); cudaFree(s->d_tw_col);
-    cudaFree(s->d_rs_in); cudaFree(s->d_rs_out);
+    cudaFree(s->d_rs_in); cudaFree(s->d_rs_out); cudaFree(s->d_rs_out32); cudaFree(s->d_W_var);
+    for (int k = 0; k < 3; ++k) cudaFree(s->d_khat_c[k]);
     cudaFree(s->d_r); cudaFree(s->d_dA); cudaFree(s->d_s2); 
     for (int k = 0; k < 2; ++k) {
         cudaFree(s->d_sigma_own[k]); cudaFree(s->d_phi_own[k]);
@@ -842,6 +966,70 @@ pg_status pg_potential_direct_rings(pg_solver *s, double *phi, int ring0, int n_
     pg_status st = potential_common(s, phi, 1, where, true, ring0, n_rings);
     s->cur_batch = saved;
     return st;
+}
+
+pg_status pg_set_softening(pg_solver *s, pg_softening mode)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (mode != PG_SOFT_SYMMETRIC && mode != PG_SOFT_FIELD && mode != PG_SOFT_SOURCE) {
+        set_err(s, "pg_set_softening: unknown mode %d", (int)mode);
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(s->device);
+    PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    if ((int)mode != s->soft) {
+        s->soft = (int)mode;
+        for (int k = 0; k < 3; ++k) s->khat_c_valid[k] = false;
+    }
+    return mode == PG_SOFT_SYMMETRIC ? PG_OK : build_khat_variant(s, 0);
+}
+
+pg_status pg_acceleration(pg_solver *s, double *a_r, double *a_phi, int batch, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!a_r || !a_phi) { set_err(s, "pg_acceleration: a_r or a_phi is NULL"); return PG_ERR_INVALID_ARG; }
+    if (s->cur_batch == 0 || !s->d_sigma) { set_err(s, "no density set: call pg_set_density first"); return PG_ERR_STATE; }
+    if (batch != s->cur_batch) {
+        set_err(s, "batch %d does not match the density's batch %d", batch, s->cur_batch);
+        return PG_ERR_INVALID_ARG;
+    }
+    if (where != PG_MEM_DEVICE && where != PG_MEM_HOST && where != PG_MEM_HOST_PINNED) {
+        set_err(s, "unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(s->device);
+    const size_t bytes = (size_t)batch * s->field * sizeof(double);
+    double *outs[2] = {a_r, a_phi};
+    if (where == PG_MEM_DEVICE) {
+        if ((((uintptr_t)a_r | (uintptr_t)a_phi) & 15u) != 0) {
+            set_err(s, "PG_MEM_DEVICE outputs must be 16-byte aligned");
+            return PG_ERR_INVALID_ARG;
+        }
+        if (ranges_overlap(a_r, bytes, a_phi, bytes) ||
+            (!s->sigma_from_host && (ranges_overlap(a_r, bytes, s->d_sigma, bytes) || ranges_overlap(a_phi, bytes, s->d_sigma, bytes)))) {
+            set_err(s, "a_r, a_phi and the density may not overlap");
+            return PG_ERR_INVALID_ARG;
+        }
+    } else {
+        // host outputs: through the owned device staging slots (two potentials' worth), blocking
+        pg_status st = ensure_staging(s, false, true);
+        if (st != PG_OK) return st;
+        PG_CUDA(s, cudaStreamSynchronize(s->d2h));
+        outs[0] = s->d_phi_own[0];
+        outs[1] = s->d_phi_own[1];
+    }
+    if (s->sigma_from_host)
+        for (int b = 0; b < batch; ++b) PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->ev_in[b], 0));
+    const int kinds[2] = {1, 2};
+    pg_status st = solve_variant(s, s->d_sigma, s->d_W, batch, 2, kinds, outs);
+    if (st != PG_OK) return st;
+    if (s->sigma_from_host) PG_CUDA(s, cudaEventRecord(s->ev_in_free[s->in_slot], s->stream));
+    if (where != PG_MEM_DEVICE) {
+        PG_CUDA(s, cudaMemcpyAsync(a_r, outs[0], bytes, cudaMemcpyDeviceToHost, s->stream));
+        PG_CUDA(s, cudaMemcpyAsync(a_phi, outs[1], bytes, cudaMemcpyDeviceToHost, s->stream));
+        PG_CUDA(s, cudaStreamSynchronize(s->stream));
+    }
+    return PG_OK;
 }
 
 pg_status pg_grid(const pg_solver *s, double *r, double *phi, double *cell_area)
