@@ -605,6 +605,24 @@ def run_staging(args):
     return 0
 
 
+def run_pipes(args):
+    """--pipes: builds and runs csrc/microbench/pipes.cu (FP64 issue rate by operand pattern, FP64 || shared-memory
+    overlap, cost of scattered 16-byte accesses) -- the measurements behind the pipe model of DESIGN.md section 7."""
+    src = os.path.join(ROOT, "paper_2409_02294_b200", "csrc", "microbench", "pipes.cu")
+    exe = os.path.join(tempfile.gettempdir(), f"pg_pipes_{os.getpid()}")
+    subprocess.run([os.environ.get("NVCC", "nvcc"), "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
+    res = subprocess.run([exe], capture_output=True, text=True)
+    os.unlink(exe)
+    out = {}
+    for line in res.stdout.splitlines():
+        t = line.split()
+        if len(t) == 3 and t[0] != "status":
+            out[t[0]] = {"value": float(t[1]), "unit": t[2]}
+    print(json.dumps({"metric": "pipe microbenchmarks (csrc/microbench/pipes.cu)", "n_gpus": 1, "results": out,
+                      "status": res.stdout.strip().splitlines()[-1] if res.stdout.strip() else res.stderr[-200:]}), flush=True)
+    return res.returncode
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -614,12 +632,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
+    ap.add_argument("--pipes", action="store_true", help="run the pipe microbenchmarks (csrc/microbench/pipes.cu)")
     ap.add_argument("--staging", action="store_true", help="time row a6 alone: pinned vs pageable staging of a 128^3 array (PAPER.md:119)")
     args = ap.parse_args()
     if args.direct:
         return run_direct(args)
     if args.staging:
         return run_staging(args)
+    if args.pipes:
+        return run_pipes(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)
