@@ -15,6 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "polar_oracle.c")
 _SRC_EXT = os.path.join(_HERE, "polar_oracle_ext.c")      # NEXT-4 variants: softening modes, acceleration
+_SRC_3D = os.path.join(_HERE, "cartesian_oracle.c")       # NEXT-2: one 3-D Cartesian mesh level
 _LIB = None
 
 
@@ -33,6 +34,8 @@ def _machine_tag() -> str:
         src = f.read()
     with open(_SRC_EXT, "rb") as f:
         src += f.read()
+    with open(_SRC_3D, "rb") as f:
+        src += f.read()
     return hashlib.sha1(flags.encode() + src).hexdigest()[:12]
 
 
@@ -46,7 +49,7 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(path):
         tmp = path + f".tmp{os.getpid()}"
         cmd = ["gcc", "-O3", "-march=native", "-fopenmp", "-fPIC", "-shared",
-               "-o", tmp, _SRC, _SRC_EXT, "-lm"]
+               "-o", tmp, _SRC, _SRC_EXT, _SRC_3D, "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(tmp, path)
     return path
@@ -64,6 +67,11 @@ def _lib():
         L.po_potential_o0_full.argtypes = [i, i, d, d, d, p, p]
         L.po_potential_o1_rings.argtypes = [i, i, d, d, d, p, p, i, p]
         L.po_potential_o1_full.argtypes = [i, i, d, d, d, p, p]
+        L.po3_self_constant.restype = d
+        L.po3_potential_targets.argtypes = [i, d, p, p, l, p]
+        L.po3_potential_full.argtypes = [i, d, p, p]
+        L.po3_potential_targets.restype = i
+        L.po3_potential_full.restype = i
         L.po_ext_o0_targets.argtypes = [i, i, d, d, d, i, p, p, l, p, p, p]
         L.po_ext_o1_rings.argtypes = [i, i, d, d, d, i, p, p, i, p, p, p]
         for fn in (L.po_grid, L.po_potential_o0_targets, L.po_potential_o0_full,
@@ -171,3 +179,30 @@ def ext_o1_rings(n_r, n_phi, r_in, r_out, eps, soft, sigma, rings):
 
 def ext_o1(n_r, n_phi, r_in, r_out, eps, soft, sigma):
     return ext_o1_rings(n_r, n_phi, r_in, r_out, eps, soft, sigma, np.arange(n_r))
+
+
+# ------------------------------------------------------------------ NEXT-2: 3-D Cartesian mesh (cartesian_oracle.c)
+def cart_self_constant() -> float:
+    return float(_lib().po3_self_constant())
+
+
+def cart_potential_targets(n, box, rho, targets):
+    """Newtonian potential (readings C1-C4) at flat target indices (z*n + y)*n + x."""
+    a = np.ascontiguousarray(rho, dtype=np.float64)
+    if a.shape != (n, n, n):
+        raise ValueError(f"rho must have shape ({n},{n},{n})")
+    t = np.ascontiguousarray(targets, dtype=np.int64)
+    if t.size and (t.min() < 0 or t.max() >= n**3):
+        raise ValueError("target index out of range")
+    out = np.empty(t.size)
+    _check(_lib().po3_potential_targets(n, box, a.ctypes.data, t.ctypes.data, t.size, out.ctypes.data), "po3_potential_targets")
+    return out
+
+
+def cart_potential(n, box, rho):
+    a = np.ascontiguousarray(rho, dtype=np.float64)
+    if a.shape != (n, n, n):
+        raise ValueError(f"rho must have shape ({n},{n},{n})")
+    out = np.empty((n, n, n))
+    _check(_lib().po3_potential_full(n, box, a.ctypes.data, out.ctypes.data), "po3_potential_full")
+    return out
