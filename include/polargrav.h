@@ -196,6 +196,32 @@ const char *pg_status_string(pg_status st);
 const char *pg_last_error(const pg_solver *s); /* s may be NULL: last error of a failed pg_create* */
 const char *pg_version(void);
 
+/* ---------------------------------------------------------------- one 3-D Cartesian mesh level
+ * The paper's own per-GPU workload: "the convolution method for solving potential fields on nested grids in three
+ * dimensions" on ONE uniform mesh level of n^3 cells, n = 64 or 128 in the paper's runs.
+ * The method's reference ([13]) is not available and PAPER.md prints no formula; readings C1-C4 of
+ * DESIGN.md section 3:
+ *     Phi_c = -G h^3 sum_{c'} rho_{c'} g(c - c'),  g(d) = 1/(h |d|) (cells as point masses), g(0) = S / h with
+ *     S = integral of 1/|x| over the unit cube = 3 ln(2 + sqrt 3) - pi/2,  G = 1,  h = box / n,
+ * over the n^3 cells of the mesh only (isolated boundary: zero padding to (2n)^3, none of which is ever stored in
+ * y or z).  Arrays are [z][y][x], x fastest, contiguous fp64; PG_MEM_DEVICE arrays 16-byte aligned.
+ *   pg3_create        n in {32, 64, 128, 256}; box > 0 is the edge length of the mesh; device -1 = current; the stream
+ *                     is borrowed.  One-time work: the real spectrum of g on the (2n)^3 lag grid.
+ *   pg3_set_density   PG_MEM_DEVICE: borrowed until the following pg3_potential has completed; host memspaces are
+ *                     copied to an owned device buffer (PG_MEM_HOST blocks until `rho` may be reused).
+ *   pg3_potential     PG_MEM_DEVICE / PG_MEM_HOST_PINNED return after enqueue; PG_MEM_HOST blocks until filled.
+ *                     `phi` may not overlap a device density.  PG_ERR_STATE before any pg3_set_density.
+ * Nested levels and their exchange across GPUs (Fig. 8) are NEXT-3 and not built. */
+typedef struct pg3_solver pg3_solver; /* opaque */
+pg_status pg3_create(pg3_solver **out, int n, double box, int device, void *cuda_stream);
+pg_status pg3_set_density(pg3_solver *s, const double *rho, pg_memspace where);
+pg_status pg3_potential(pg3_solver *s, double *phi, pg_memspace where);
+pg_status pg3_synchronize(pg3_solver *s);
+pg_status pg3_destroy(pg3_solver *s); /* pg3_destroy(NULL) is a no-op returning PG_OK */
+long pg3_launch_count(const pg3_solver *s);
+double pg3_algorithmic_bytes(const pg3_solver *s);
+const char *pg3_last_error(const pg3_solver *s); /* s may be NULL: last error of a failed pg3_create */
+
 #ifdef __cplusplus
 }
 #endif

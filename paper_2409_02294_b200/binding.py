@@ -29,6 +29,8 @@ EXPORTS = (
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
     "pg_version", "pg_set_softening", "pg_acceleration",
+    "pg3_create", "pg3_set_density", "pg3_potential", "pg3_synchronize", "pg3_destroy", "pg3_launch_count",
+    "pg3_algorithmic_bytes", "pg3_last_error",
 )
 
 _lib = None
@@ -67,8 +69,16 @@ def lib():
         L.pg_host_free.argtypes = [vp]
         L.pg_profile.argtypes = [vp, i]
         L.pg_kernel_times.argtypes = [vp, ctypes.POINTER(d), ctypes.POINTER(l)]
+        L.pg3_create.argtypes = [ctypes.POINTER(vp), i, d, i, vp]
+        L.pg3_set_density.argtypes = [vp, vp, i]
+        L.pg3_potential.argtypes = [vp, vp, i]
+        L.pg3_synchronize.argtypes = [vp]
+        L.pg3_destroy.argtypes = [vp]
         for name in EXPORTS:
             getattr(L, name).restype = i
+        L.pg3_launch_count.argtypes = [vp]; L.pg3_launch_count.restype = l
+        L.pg3_algorithmic_bytes.argtypes = [vp]; L.pg3_algorithmic_bytes.restype = d
+        L.pg3_last_error.argtypes = [vp]; L.pg3_last_error.restype = ctypes.c_char_p
         L.pg_launch_count.argtypes = [vp]; L.pg_launch_count.restype = l
         L.pg_algorithmic_bytes.argtypes = [vp, i]; L.pg_algorithmic_bytes.restype = d
         L.pg_kernel_algorithmic_bytes.argtypes = [vp, i, i]; L.pg_kernel_algorithmic_bytes.restype = d
@@ -202,6 +212,47 @@ def pg_algorithmic_bytes(h, batch=1):
 
 def pg_kernel_algorithmic_bytes(h, index, batch=1):
     return float(lib().pg_kernel_algorithmic_bytes(h, index, batch))
+
+
+# ------------------------------------------------------------------ NEXT-2: 3-D Cartesian mesh level
+def _check3(st, handle=None):
+    if st != PG_OK:
+        msg = lib().pg3_last_error(handle).decode()
+        raise PolargravError(st, f"{status_string(st)}: {msg}")
+
+
+def pg3_create(n, box, device=-1, cuda_stream=None):
+    h = ctypes.c_void_p()
+    _check3(lib().pg3_create(ctypes.byref(h), n, box, device, ctypes.c_void_p(cuda_stream) if cuda_stream else None))
+    return h
+
+
+def pg3_set_density(h, rho, where):
+    _check3(lib().pg3_set_density(h, _ptr(rho), where), h)
+
+
+def pg3_potential(h, phi, where):
+    _check3(lib().pg3_potential(h, _ptr(phi), where), h)
+
+
+def pg3_synchronize(h):
+    _check3(lib().pg3_synchronize(h), h)
+
+
+def pg3_destroy(h):
+    _check3(lib().pg3_destroy(h))
+
+
+def pg3_launch_count(h):
+    return int(lib().pg3_launch_count(h))
+
+
+def pg3_algorithmic_bytes(h):
+    return float(lib().pg3_algorithmic_bytes(h))
+
+
+def pg3_last_error(h=None):
+    return lib().pg3_last_error(h).decode()
 
 
 # ------------------------------------------------------------------ convenience wrapper

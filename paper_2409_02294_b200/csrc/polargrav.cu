@@ -7,6 +7,7 @@
 #include "../../include/polargrav.h"
 #include "kernels.cuh"
 #include "variants.cuh"
+#include "cartesian.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -1155,5 +1156,271 @@ const char *pg_status_string(pg_status st)
 const char *pg_last_error(const pg_solver *s) { return s ? s->err : g_create_error; }
 
 const char *pg_version(void) { return "polargrav 0.1 (sm_100a)"; }
+
+}  // extern "C"
+
+// =================================================================== NEXT-2: one 3-D Cartesian mesh level
+struct pg3_solver {
+    int n = 0, device = 0;
+    double box = 0, h = 0;
+    pg_solver *inner = nullptr;      // tables, stream and launch helpers of a polar solver with n_r = n, n_phi = 2 n
+    double *d_P = nullptr;           // [n*n rows][2n] reals: x zero padded / inverse x pass
+    cplx *d_Yt = nullptr;            // [n+1][2n][n]: spectrum after the x and y passes, z contiguous
+    double *d_ghat = nullptr;        // [n+1][2n][2n] real spectrum of the Green's function (all normalisations folded in)
+    double *d_ones = nullptr;        // post-scale of the inverse x pass (none)
+    double *d_rho = nullptr, *d_phi = nullptr;   // staging for host memspaces (lazily allocated)
+    const double *cur_rho = nullptr;
+    bool rho_from_host = false;
+    char err[512] = "";
+};
+
+namespace {
+
+void set_err3(pg3_solver *s, const char *fmt, ...)
+{
+    char *dst = s ? s->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+}
+#define PG3_CUDA(s, call)                                                                      \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            set_err3((s), "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return e_ == cudaErrorMemoryAllocation ? PG_ERR_NOMEM : PG_ERR_CUDA;               \
+        }                                                                                      \
+    } while (0)
+
+template <int N>
+pg_status cart_build_ghat(pg3_solver *s)
+{
+    typedef pgk::ColShape<N> S;
+    constexpr int M = 2 * N;
+    pg_solver *in = s->inner;
+    cudaStream_t st = in->stream;
+    const long g_n = (long)M * M * M, gw_n = (long)M * (N + 1) * M;
+    double *d_g = nullptr;
+    cplx *d_gw = nullptr, *d_gy = nullptr;
+    PG3_CUDA(s, cudaMalloc((void **)&d_g, g_n * sizeof(double)));
+    if (cudaMalloc((void **)&d_gw, gw_n * sizeof(cplx)) != cudaSuccess || cudaMalloc((void **)&d_gy, gw_n * sizeof(cplx)) != cudaSuccess) {
+        cudaFree(d_g); cudaFree(d_gw); cudaFree(d_gy);
+        set_err3(s, "out of device memory for the Green's function workspace");
+        return PG_ERR_NOMEM;
+    }
+    pg_status rc = PG_OK;
+    do {
+        const double self = 3.0 * std::log(2.0 + std::sqrt(3.0)) - 2.0 * std::atan(1.0);      // reading C3
+        pgk::green3_fill_kernel<<<(unsigned)((g_n + 255) / 256), 256, 0, st>>>(d_g, N, self, g_n);
+        // x' pass: the 2N x 2N rows as 2N fields of 2N rows -> GW[z'][kx][y']
+        rc = rows_fwd(in, d_g, d_gw, nullptr, M, M, (long)M * M, (long)(N + 1) * M, st, 0);
+        if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", in->err); break; }
+        const size_t smem = S::LINES;
+        cudaFuncSetAttribute(pgk::gcols_kernel<N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaFuncSetAttribute(pgk::gcols_kernel<N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const int n_cols = M * (N + 1);
+        const unsigned grid = (unsigned)((n_cols + S::MODES - 1) / S::MODES);
+        // -G h^2 (cells as point masses: h^3 / h), and the normalisation of the unnormalised transforms: x pair 1/(2M)
+        // (packed real transform: 2 X on the way in, 2 Z on the way out) and another 1/2 because the kernel's own x'
+        // pass forms 2 X; y and z pairs 1/M each.
+        const double scale = -s->h * s->h / (4.0 * (double)M * (double)M * (double)M);
+        pgk::gcols_kernel<N, 0><<<grid, S::THREADS, smem, st>>>(d_gw, d_gy, nullptr, in->d_tw_col, n_cols, 0.0);
+        pgk::gcols_kernel<N, 1><<<grid, S::THREADS, smem, st>>>(d_gy, nullptr, s->d_ghat, in->d_tw_col, n_cols, scale);
+        in->launches += 3;
+        if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+            set_err3(s, "Green's function precompute failed: %s", cudaGetErrorString(cudaGetLastError()));
+            rc = PG_ERR_CUDA;
+        }
+    } while (0);
+    cudaFree(d_g); cudaFree(d_gw); cudaFree(d_gy);
+    return rc;
+}
+
+template <int N>
+pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
+{
+    typedef pgk::ColShape<N> S;
+    constexpr int M = 2 * N;
+    pg_solver *in = s->inner;
+    cudaStream_t st = in->stream;
+    const long p_n = (long)N * N * M, f_n = (long)N * N * N, ws = (long)(N + 1) * N;
+    pgk::pad3_kernel<<<(unsigned)((p_n + 255) / 256), 256, 0, st>>>(d_rho, s->d_P, N, p_n);
+    in->launches++;
+    // x pass: N fields (z) of N rows (y) of M reals -> W1[z][kx][y]
+    pg_status rc = rows_fwd(in, s->d_P, in->d_W, nullptr, N, N, (long)N * M, ws, st, 0);
+    if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", in->err); return rc; }
+    const int n_cols = N * (N + 1);
+    const unsigned ygrid = (unsigned)((n_cols + S::MODES - 1) / S::MODES);
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_fwd_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::LINES));
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_inv_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::LINES));
+    pgk::ycols_fwd_kernel<N><<<ygrid, S::THREADS, S::LINES, st>>>(in->d_W, s->d_Yt, in->d_tw_col, n_cols);
+    in->launches++;
+    // z pass: cols_kernel unchanged -- zero-padded 2N-point transform x Ghat, inverse, crop -- over the (N+1) 2N columns
+    const int n_modes = (N + 1) * M;
+    dim3 zgrid((n_modes + S::MODES - 1) / S::MODES, 1);
+    PG3_CUDA(s, launch_pdl(pgk::cols_kernel<N>, zgrid, dim3(S::THREADS), S::SMEM, st, s->d_Yt, (const double *)s->d_ghat,
+                           (const cplx *)in->d_tw_col, n_modes, 0L));
+    in->launches++;
+    pgk::ycols_inv_kernel<N><<<ygrid, S::THREADS, S::LINES, st>>>(s->d_Yt, in->d_W, in->d_tw_col, n_cols);
+    in->launches++;
+    rc = rows_inv(in, in->d_W, s->d_P, N, ws, (long)N * M, st, s->d_ones);
+    if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", in->err); return rc; }
+    pgk::crop3_kernel<<<(unsigned)((f_n + 255) / 256), 256, 0, st>>>(s->d_P, d_phi, N, f_n);
+    in->launches++;
+    PG3_CUDA(s, cudaGetLastError());
+    return PG_OK;
+}
+
+#define PG3_DISPATCH(n, CALL)                          \
+    switch (n) {                                        \
+        case 32: return CALL(32);                       \
+        case 64: return CALL(64);                       \
+        case 128: return CALL(128);                     \
+        case 256: return CALL(256);                     \
+        default: return PG_ERR_UNSUPPORTED;             \
+    }
+pg_status cart_build(pg3_solver *s)
+{
+#define CALL(N) cart_build_ghat<N>(s)
+    PG3_DISPATCH(s->n, CALL)
+#undef CALL
+}
+pg_status cart_run(pg3_solver *s, const double *d_rho, double *d_phi)
+{
+#define CALL(N) cart_solve<N>(s, d_rho, d_phi)
+    PG3_DISPATCH(s->n, CALL)
+#undef CALL
+}
+
+void cart_free(pg3_solver *s)
+{
+    if (!s) return;
+    cudaFree(s->d_P); cudaFree(s->d_Yt); cudaFree(s->d_ghat); cudaFree(s->d_ones); cudaFree(s->d_rho); cudaFree(s->d_phi);
+    if (s->inner) pg_destroy(s->inner);
+    delete s;
+}
+
+}  // namespace
+
+extern "C" {
+
+pg_status pg3_create(pg3_solver **out, int n, double box, int device, void *cuda_stream)
+{
+    g_create_error[0] = 0;
+    if (!out) { set_err3(nullptr, "out is NULL"); return PG_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!(box > 0.0) || !std::isfinite(box)) { set_err3(nullptr, "invalid argument: need box > 0"); return PG_ERR_INVALID_ARG; }
+    if (n != 32 && n != 64 && n != 128 && n != 256) {
+        set_err3(nullptr, "unsupported mesh %d^3: n must be 32, 64, 128 or 256", n);
+        return PG_ERR_UNSUPPORTED;
+    }
+    pg3_solver *s = new (std::nothrow) pg3_solver;
+    if (!s) { set_err3(nullptr, "out of host memory"); return PG_ERR_NOMEM; }
+    s->n = n; s->box = box; s->h = box / n;
+    // tables (twiddles of the 2n-point transforms), stream and workspace W1 = [n][n+1][n] come with a polar solver of
+    // n_r = n, n_phi = 2n, max_batch = n; its own Green's kernel is not used
+    pg_status rc = pg_create_ex(&s->inner, n, 2 * n, 1.0, 2.0, 1.0, n, device, cuda_stream);
+    if (rc != PG_OK) { delete s; return rc; }
+    s->device = s->inner->device;
+    DeviceGuard guard(s->device);
+    const size_t m = 2 * (size_t)n;
+    std::vector<double> ones(n, 1.0);
+    cudaError_t e = cudaMalloc((void **)&s->d_P, (size_t)n * n * m * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_Yt, (size_t)(n + 1) * m * n * sizeof(cplx));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_ghat, (size_t)(n + 1) * m * m * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_ones, n * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(s->d_ones, ones.data(), n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        set_err3(nullptr, "device allocation failed: %s", cudaGetErrorString(e));
+        cart_free(s);
+        return PG_ERR_NOMEM;
+    }
+    rc = cart_build(s);
+    if (rc != PG_OK) {
+        snprintf(g_create_error, sizeof g_create_error, "%s", s->err);
+        cart_free(s);
+        return rc;
+    }
+    *out = s;
+    return PG_OK;
+}
+
+pg_status pg3_set_density(pg3_solver *s, const double *rho, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!rho) { set_err3(s, "pg3_set_density: rho is NULL"); return PG_ERR_INVALID_ARG; }
+    DeviceGuard guard(s->device);
+    const size_t bytes = (size_t)s->n * s->n * s->n * sizeof(double);
+    if (where == PG_MEM_DEVICE) {
+        if (((uintptr_t)rho & 15u) != 0) { set_err3(s, "a PG_MEM_DEVICE density must be 16-byte aligned"); return PG_ERR_INVALID_ARG; }
+        s->cur_rho = rho;
+        s->rho_from_host = false;
+    } else if (where == PG_MEM_HOST || where == PG_MEM_HOST_PINNED) {
+        if (!s->d_rho) PG3_CUDA(s, cudaMalloc((void **)&s->d_rho, bytes));
+        PG3_CUDA(s, cudaMemcpyAsync(s->d_rho, rho, bytes, cudaMemcpyHostToDevice, s->inner->stream));
+        if (where == PG_MEM_HOST) PG3_CUDA(s, cudaStreamSynchronize(s->inner->stream));
+        s->cur_rho = s->d_rho;
+        s->rho_from_host = true;
+    } else {
+        set_err3(s, "pg3_set_density: unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    return PG_OK;
+}
+
+pg_status pg3_potential(pg3_solver *s, double *phi, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!phi) { set_err3(s, "pg3_potential: phi is NULL"); return PG_ERR_INVALID_ARG; }
+    if (!s->cur_rho) { set_err3(s, "no density set: call pg3_set_density first"); return PG_ERR_STATE; }
+    DeviceGuard guard(s->device);
+    const size_t bytes = (size_t)s->n * s->n * s->n * sizeof(double);
+    if (where == PG_MEM_DEVICE) {
+        if (((uintptr_t)phi & 15u) != 0) { set_err3(s, "a PG_MEM_DEVICE potential must be 16-byte aligned"); return PG_ERR_INVALID_ARG; }
+        if (!s->rho_from_host && ranges_overlap(phi, bytes, s->cur_rho, bytes)) {
+            set_err3(s, "phi overlaps the density");
+            return PG_ERR_INVALID_ARG;
+        }
+        return cart_run(s, s->cur_rho, phi);
+    }
+    if (where != PG_MEM_HOST && where != PG_MEM_HOST_PINNED) { set_err3(s, "unknown memspace %d", (int)where); return PG_ERR_INVALID_ARG; }
+    if (!s->d_phi) PG3_CUDA(s, cudaMalloc((void **)&s->d_phi, bytes));
+    pg_status rc = cart_run(s, s->cur_rho, s->d_phi);
+    if (rc != PG_OK) return rc;
+    PG3_CUDA(s, cudaMemcpyAsync(phi, s->d_phi, bytes, cudaMemcpyDeviceToHost, s->inner->stream));
+    if (where == PG_MEM_HOST) PG3_CUDA(s, cudaStreamSynchronize(s->inner->stream));
+    return PG_OK;
+}
+
+pg_status pg3_synchronize(pg3_solver *s)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    return pg_synchronize(s->inner);
+}
+
+pg_status pg3_destroy(pg3_solver *s)
+{
+    if (!s) return PG_OK;
+    DeviceGuard guard(s->device);
+    cudaStreamSynchronize(s->inner->stream);
+    cart_free(s);
+    return PG_OK;
+}
+
+long pg3_launch_count(const pg3_solver *s) { return s ? s->inner->launches : 0; }
+
+const char *pg3_last_error(const pg3_solver *s) { return s ? s->err : g_create_error; }
+
+/* Algorithmic HBM bytes of one pg3_potential call: rho in, Phi out, and each intermediate
+ * spectrum written and read once at its pruned size -- x pass out / y pass in (n+1) n^2, y pass out / z pass in-out /
+ * y pass in (n+1) 2n n, complex128 -- plus the real Green's spectrum (n+1)(2n)^2 once. */
+double pg3_algorithmic_bytes(const pg3_solver *s)
+{
+    if (!s) return 0.0;
+    const double n = s->n, cells = n * n * n;
+    const double w1 = 16.0 * (n + 1) * n * n, yt = 16.0 * (n + 1) * 2.0 * n * n, gh = 8.0 * (n + 1) * 4.0 * n * n;
+    return 2.0 * 8.0 * cells + 2.0 * w1 + 2.0 * w1 + 4.0 * yt + gh;
+}
 
 }  // extern "C"

@@ -16,7 +16,7 @@ HEADER = os.path.join(ROOT, "include", "polargrav.h")
 def declared_functions():
     src = open(HEADER).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(pg_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(pg3?_[a-z_]+)\s*\(", src)))
 
 
 @pytest.fixture(scope="module")
@@ -41,7 +41,7 @@ def test_binding_has_the_same_names(lib):
     names = declared_functions()
     assert sorted(binding.EXPORTS) == names
     for name in names:
-        if name in ("pg_status_string", "pg_last_error", "pg_version"):
+        if name in ("pg_status_string", "pg_last_error", "pg_version", "pg3_last_error"):
             continue
         assert callable(getattr(binding, name)), name
 
@@ -69,6 +69,15 @@ def test_argument_validation_needs_no_gpu(lib):
     assert e.value.status == binding.PG_ERR_UNSUPPORTED
     assert binding.lib().pg_destroy(None) == binding.PG_OK   # no-op
     assert binding.lib().pg_set_density(None, None, 1, 0) == binding.PG_ERR_INVALID_ARG
+    # the 3-D mesh calls (NEXT-2)
+    with pytest.raises(binding.PolargravError) as e:
+        binding.pg3_create(48, 1.0)                          # not a supported mesh size
+    assert e.value.status == binding.PG_ERR_UNSUPPORTED
+    with pytest.raises(binding.PolargravError) as e:
+        binding.pg3_create(64, 0.0)                          # box <= 0
+    assert e.value.status == binding.PG_ERR_INVALID_ARG
+    assert binding.lib().pg3_destroy(None) == binding.PG_OK
+    assert binding.lib().pg3_set_density(None, None, 0) == binding.PG_ERR_INVALID_ARG
 
 
 def test_no_cpu_fallback_without_a_device(lib):
