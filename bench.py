@@ -605,6 +605,130 @@ def run_staging(args):
     return 0
 
 
+def make_rho3(n: int, seed: int):
+    """Synthetic mesh level in the spirit of the paper's runs, whose contents are never described:
+    a centrally condensed clump, six seeded Gaussian clumps, 1 % noise; non-negative.  (Same recipe as
+    tests/test_gpu_cartesian.py.)"""
+    rng = np.random.Generator(np.random.PCG64(2409022940 + 1000 * n + seed))
+    z, y, x = np.meshgrid(*(np.arange(n) + 0.5,) * 3, indexing="ij")
+    c = n / 2.0
+    rho = 1.0 / (1.0 + ((x - c) ** 2 + (y - c) ** 2 + (z - c) ** 2) / (0.1 * n) ** 2)
+    for _ in range(6):
+        cx, cy, cz = rng.uniform(0.2 * n, 0.8 * n, 3)
+        w = rng.uniform(1.5, 4.0)
+        rho += rng.uniform(0.5, 3.0) * np.exp(-((x - cx) ** 2 + (y - cy) ** 2 + (z - cz) ** 2) / (2 * w * w))
+    return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))
+
+
+def run_cart(args):
+    """--cart N: the paper's own per-GPU workload (row NEXT-2): potential of ONE 3-D Cartesian mesh level of N^3 cells
+    (N = 64 or 128) by the zero-padded FFT convolution, device resident.  Same protocol as the main
+    line: median of REPEATS repeats of the K-step region, buffer rotation beyond L2, parity gate against the 3-D oracle
+    on sampled cells, oracle timed on the host cores.  Not the headline metric (BASELINE.json's is the 2-D path)."""
+    import torch
+    import oracle
+    from paper_2409_02294_b200 import binding as pg, build as pg_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    n, box = args.cart, 10.0
+    st = torch.cuda.Stream()
+    h = pg.pg3_create(n, box, 0, st.cuda_stream)
+    field_bytes = 8 * n**3
+    R = int(min(64, max(4, -(-4 * L2_BYTES // (2 * field_bytes)))))
+    base = [make_rho3(n, k) for k in range(min(R, 4))]
+    d_rho = [torch.from_numpy(np.roll(base[k % len(base)], 7 * (k // len(base)), axis=2)).cuda() for k in range(R)]
+    d_phi = [torch.empty_like(d_rho[0]) for _ in range(R)]
+    torch.cuda.synchronize()
+
+    def step(k):
+        pg.pg3_set_density(h, d_rho[k % R], pg.PG_MEM_DEVICE)
+        pg.pg3_potential(h, d_phi[k % R], pg.PG_MEM_DEVICE)
+
+    for k in range(max(3, args.warmup)):
+        step(k)
+    pg.pg3_synchronize(h)
+    sampler = ClockSampler(0)
+    rep_ms = []
+    n0 = pg.pg3_launch_count(h)
+    for _ in range(REPEATS):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(st)
+        for k in range(args.steps):
+            step(k)
+        e1.record(st)
+        torch.cuda.synchronize()
+        rep_ms.append(e0.elapsed_time(e1))
+    n1 = pg.pg3_launch_count(h)
+    got = d_phi[0].cpu().numpy()
+    t_end = time.perf_counter() + 0.6
+    k = 0
+    while time.perf_counter() < t_end:
+        step(k); k += 1
+        if k % 64 == 0:
+            pg.pg3_synchronize(h)
+    pg.pg3_synchronize(h)
+    clocks = sampler.stop()
+    ms_per_step = float(np.median(rep_ms)) / args.steps
+    # parity gate + oracle timing on a bounded sample of target cells
+    rng = np.random.default_rng(n)
+    n_t = {32: 4096, 64: 4096, 128: 1024, 256: 128}[n]
+    tg = np.unique(np.concatenate([[0, n**3 - 1], rng.integers(0, n**3, n_t)])).astype(np.int64)
+    t0 = time.perf_counter()
+    ref = oracle.cart_potential_targets(n, box, base[0], tg)
+    t_or = time.perf_counter() - t0
+    l2 = float(np.linalg.norm(got.reshape(-1)[tg] - ref) / np.linalg.norm(ref))
+    mx = float(np.abs(got.reshape(-1)[tg] / ref - 1.0).max())
+    ok = bool(l2 <= REL_L2 and mx <= MAX_REL)
+    peak, peak_src = load_peaks()
+    alg = pg.pg3_algorithmic_bytes(h)
+    gbs = alg / (ms_per_step * 1e-3) / 1e9
+    # end to end with pinned host buffers
+    pin_in, pin_out = pg.PinnedArray((n, n, n)), pg.PinnedArray((n, n, n))
+    pin_in.array[...] = base[0]
+    for _ in range(3):
+        pg.pg3_set_density(h, pin_in.ptr, pg.PG_MEM_HOST_PINNED); pg.pg3_potential(h, pin_out.ptr, pg.PG_MEM_HOST_PINNED)
+    pg.pg3_synchronize(h)
+    e2e_steps = max(3, min(args.steps, 20))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        pg.pg3_set_density(h, pin_in.ptr, pg.PG_MEM_HOST_PINNED); pg.pg3_potential(h, pin_out.ptr, pg.PG_MEM_HOST_PINNED)
+    pg.pg3_synchronize(h)
+    t_e2e = (time.perf_counter() - t0) / e2e_steps
+    line = {
+        "metric": "potential solves/sec (fp64 zero-padded FFT convolution, one 3-D Cartesian mesh level; row NEXT-2)",
+        "value": 1e3 / ms_per_step, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"one {n}^3 Cartesian mesh level (PAPER.md:267, :271), box {box:g}, isolated boundary, "
+                               "condensed clump + 6 Gaussian clumps + 1 % noise", "n": n,
+                   "l2": f"inputs larger than L2: steps rotate over {R} (rho, Phi) buffer pairs"},
+        "cells_per_s": n**3 * 1e3 / ms_per_step, "gpu_launches": int(round((n1 - n0) / REPEATS)),
+        "repeats": {"n": REPEATS, "ms_per_step_median": ms_per_step, "ms_per_step_min": min(rep_ms) / args.steps,
+                    "ms_per_step_max": max(rep_ms) / args.steps},
+        "parity": {"rel_l2": l2, "max_rel": mx, "cells": int(len(tg)), "bar": {"rel_l2": REL_L2, "max_rel": MAX_REL}, "ok": ok,
+                   "what": "Phi of buffer 0 as the timed region left it vs oracle/cartesian_oracle.c on sampled cells"},
+        "roofline": {"bound": "hbm", "kernel": "whole path (7 launches)", "achieved": gbs, "peak": peak, "unit": "GB/s",
+                     "frac": gbs / peak, "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_step": alg},
+        "e2e": {"value": 1.0 / t_e2e, "unit": UNIT, "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes,
+                "how": "pg3_set_density + pg3_potential with PG_MEM_HOST_PINNED buffers, wall clock, pg3_synchronize at the end"},
+        "clocks": clocks,
+        "cpu_baseline": {"value": (len(tg) / n**3) / t_or, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": f"oracle/cartesian_oracle.c (direct sum, gcc -O3 -march=native -fopenmp) on {len(tg)} of {n**3} "
+                                   f"target cells ({t_or:.2f} s), extrapolated to the whole mesh by cells"},
+        "host": host_placement(0),
+    }
+    pin_in.free(); pin_out.free()
+    pg.pg3_destroy(h)
+    print(json.dumps(line), flush=True)
+    if not ok:
+        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {line['parity']}\n")
+        return 3
+    return 0
+
+
 def run_pipes(args):
     """--pipes: builds and runs csrc/microbench/pipes.cu (FP64 issue rate by operand pattern, FP64 || shared-memory
     overlap, cost of scattered 16-byte accesses) -- the measurements behind the pipe model of DESIGN.md section 7."""
@@ -632,6 +756,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
+    ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
+                    help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")
     ap.add_argument("--pipes", action="store_true", help="run the pipe microbenchmarks (csrc/microbench/pipes.cu)")
     ap.add_argument("--staging", action="store_true", help="time row a6 alone: pinned vs pageable staging of a 128^3 array (PAPER.md:119)")
     args = ap.parse_args()
@@ -641,6 +767,8 @@ def main():
         return run_staging(args)
     if args.pipes:
         return run_pipes(args)
+    if args.cart:
+        return run_cart(args)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     return run_reference(args) if args.impl == "reference" else run_ours(args)
