@@ -263,7 +263,9 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // real-data split run with thread = (t, row) and the ROW fastest, so that the modes W[m][i] leave as
 // runs of ROWS consecutive rows of one column: the transposed store costs no extra shared-memory
 // round trip.
-template <int NPHI>
+// HALF (the x pass of the 3-D mesh path, cartesian.cuh): the rows in memory hold only the first n_phi/2 reals, the
+// second half of the transform's input is zero padding that is never read.
+template <int NPHI, bool HALF = false>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
                 const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
@@ -292,9 +294,9 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
 
     auto prefetch = [&](const int item) {
         const int f = item / items_per_field, i = (item % items_per_field) * ROWS + rho;
-        const cplx *x = reinterpret_cast<const cplx *>(sigma + f * sigma_field_stride + (long)i * NPHI) + u;
+        const cplx *x = reinterpret_cast<const cplx *>(sigma + f * sigma_field_stride + (long)i * (HALF ? NPHI / 2 : NPHI)) + u;
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) cp_async16(stage + jj * S::THREADS, x + T * jj);
+        for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) cp_async16(stage + jj * S::THREADS, x + T * jj);
         cp_async_commit();
     };
 
@@ -322,7 +324,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         sc_next = row_scale(item + gridDim.x);
         cp_async_wait_all();
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) v[jj] = stage[jj * S::THREADS];
+        for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage[jj * S::THREADS];
         if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
         if (rscale != nullptr) {
 #pragma unroll
@@ -351,7 +353,8 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
 // mapping (transposed access in runs of ROWS rows), re-packs them into the spectrum of the packed
 // row, inverse pass C; the remaining passes with u fastest; multiplies row i by oscale_i
 // (= r_i^{-1/2}) and stores Phi_i.
-template <int NPHI>
+// HALF: only the first n_phi/2 reals of every output row are stored, in rows of that length (the crop of the x pass).
+template <int NPHI, bool HALF = false>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
                 const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
@@ -409,9 +412,9 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
             sync();
         }
         inv_a<L, ROW>(v, line, bases, u);
-        cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * NPHI);
+        cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * (HALF ? NPHI / 2 : NPHI));
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
+        for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
         __syncthreads();   // the lines are rewritten by the next item's pass C
     }
 }

@@ -1164,7 +1164,6 @@ struct pg3_solver {
     int n = 0, device = 0;
     double box = 0, h = 0;
     pg_solver *inner = nullptr;      // tables, stream and launch helpers of a polar solver with n_r = n, n_phi = 2 n
-    double *d_P = nullptr;           // [n*n rows][2n] reals: x zero padded / inverse x pass
     cplx *d_Yt = nullptr;            // [n+1][2n][n]: spectrum after the x and y passes, z contiguous
     double *d_ghat = nullptr;        // [n+1][2n][2n] real spectrum of the Green's function (all normalisations folded in)
     double *d_ones = nullptr;        // post-scale of the inverse x pass (none)
@@ -1244,17 +1243,21 @@ pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
     constexpr int M = 2 * N;
     pg_solver *in = s->inner;
     cudaStream_t st = in->stream;
-    const long p_n = (long)N * N * M, f_n = (long)N * N * N, ws = (long)(N + 1) * N;
-    pgk::pad3_kernel<<<(unsigned)((p_n + 255) / 256), 256, 0, st>>>(d_rho, s->d_P, N, p_n);
+    const long ws = (long)(N + 1) * N;
+    typedef pgk::RowShape<M> RS;
+    const int n_items = (N / RS::ROWS) * N;
+    const int rgrid = n_items < in->row_ctas ? n_items : in->row_ctas;
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::rows_fwd_kernel<M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::SMEM));
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::rows_inv_kernel<M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS::SMEM));
+    // x pass: N fields (z) of N rows (y) of N reals, zero padded to M inside the kernel -> W1[z][kx][y]
+    PG3_CUDA(s, launch_pdl(pgk::rows_fwd_kernel<M, true>, dim3(rgrid), dim3(RS::THREADS), RS::SMEM, st, d_rho, in->d_W,
+                           (const cplx *)in->d_tw_row, (const double *)nullptr, N, n_items, (long)N * N, ws, 0));
     in->launches++;
-    // x pass: N fields (z) of N rows (y) of M reals -> W1[z][kx][y]
-    pg_status rc = rows_fwd(in, s->d_P, in->d_W, nullptr, N, N, (long)N * M, ws, st, 0);
-    if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", in->err); return rc; }
-    const int n_cols = N * (N + 1);
-    const unsigned ygrid = (unsigned)((n_cols + S::MODES - 1) / S::MODES);
-    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_fwd_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::LINES));
-    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_inv_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::LINES));
-    pgk::ycols_fwd_kernel<N><<<ygrid, S::THREADS, S::LINES, st>>>(in->d_W, s->d_Yt, in->d_tw_col, n_cols);
+    typedef pgk::YShape<N> Y;
+    const unsigned ygrid = (unsigned)((N + 1) * N / Y::YM);
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_fwd_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Y::SMEM));
+    PG3_CUDA(s, cudaFuncSetAttribute(pgk::ycols_inv_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Y::SMEM));
+    pgk::ycols_fwd_kernel<N><<<ygrid, Y::THREADS, Y::SMEM, st>>>(in->d_W, s->d_Yt, in->d_tw_col);
     in->launches++;
     // z pass: cols_kernel unchanged -- zero-padded 2N-point transform x Ghat, inverse, crop -- over the (N+1) 2N columns
     const int n_modes = (N + 1) * M;
@@ -1262,11 +1265,11 @@ pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
     PG3_CUDA(s, launch_pdl(pgk::cols_kernel<N>, zgrid, dim3(S::THREADS), S::SMEM, st, s->d_Yt, (const double *)s->d_ghat,
                            (const cplx *)in->d_tw_col, n_modes, 0L));
     in->launches++;
-    pgk::ycols_inv_kernel<N><<<ygrid, S::THREADS, S::LINES, st>>>(s->d_Yt, in->d_W, in->d_tw_col, n_cols);
+    pgk::ycols_inv_kernel<N><<<ygrid, Y::THREADS, Y::SMEM, st>>>(s->d_Yt, in->d_W, in->d_tw_col);
     in->launches++;
-    rc = rows_inv(in, in->d_W, s->d_P, N, ws, (long)N * M, st, s->d_ones);
-    if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", in->err); return rc; }
-    pgk::crop3_kernel<<<(unsigned)((f_n + 255) / 256), 256, 0, st>>>(s->d_P, d_phi, N, f_n);
+    // inverse x pass, cropped to the first N reals of every row: Phi[z][y][x]
+    PG3_CUDA(s, launch_pdl(pgk::rows_inv_kernel<M, true>, dim3(rgrid), dim3(RS::THREADS), RS::SMEM, st, (const cplx *)in->d_W,
+                           d_phi, (const cplx *)in->d_tw_row, (const double *)s->d_ones, N, n_items, ws, (long)N * N));
     in->launches++;
     PG3_CUDA(s, cudaGetLastError());
     return PG_OK;
@@ -1296,7 +1299,7 @@ pg_status cart_run(pg3_solver *s, const double *d_rho, double *d_phi)
 void cart_free(pg3_solver *s)
 {
     if (!s) return;
-    cudaFree(s->d_P); cudaFree(s->d_Yt); cudaFree(s->d_ghat); cudaFree(s->d_ones); cudaFree(s->d_rho); cudaFree(s->d_phi);
+    cudaFree(s->d_Yt); cudaFree(s->d_ghat); cudaFree(s->d_ones); cudaFree(s->d_rho); cudaFree(s->d_phi);
     if (s->inner) pg_destroy(s->inner);
     delete s;
 }
@@ -1326,8 +1329,7 @@ pg_status pg3_create(pg3_solver **out, int n, double box, int device, void *cuda
     DeviceGuard guard(s->device);
     const size_t m = 2 * (size_t)n;
     std::vector<double> ones(n, 1.0);
-    cudaError_t e = cudaMalloc((void **)&s->d_P, (size_t)n * n * m * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_Yt, (size_t)(n + 1) * m * n * sizeof(cplx));
+    cudaError_t e = cudaMalloc((void **)&s->d_Yt, (size_t)(n + 1) * m * n * sizeof(cplx));
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_ghat, (size_t)(n + 1) * m * m * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_ones, n * sizeof(double));
     if (e == cudaSuccess) e = cudaMemcpy(s->d_ones, ones.data(), n * sizeof(double), cudaMemcpyHostToDevice);
