@@ -273,6 +273,10 @@ def run_ours(args):
     h = solver.h
     # the densities of the timed loop are resident in HBM and complete before the loop starts
     pg.pg_set_option(h, pg.PG_OPT_DENSITY_STABLE, 1)
+    # the solves of the timed loop are independent (distinct resident buffer pairs): two in flight (PG_OPT_LANES),
+    # joined into the timing stream by pg_flush before the end event.  Off for the host-bound small grids.
+    lanes = args.lanes if args.lanes else (2 if c.n_r * c.n_phi >= 1 << 20 else 1)
+    pg.pg_set_option(h, pg.PG_OPT_LANES, lanes)
     r, phi, _ = solver.grid()
     n_fields = R * c.batch
     distinct = min(n_fields, 8 if c.n_r * c.n_phi >= 1 << 22 else 32)
@@ -310,6 +314,7 @@ def run_ours(args):
         e0.record(st)
         for k in range(args.steps):
             step(k)
+        pg.pg_flush(h)
         e1.record(st)
         torch.cuda.synchronize(); barrier()
         rep_ms.append(max_over_ranks(e0.elapsed_time(e1)))
@@ -357,7 +362,9 @@ def run_ours(args):
     path_bytes = pg.pg_algorithmic_bytes(h, c.batch)
     path_gbs = path_bytes / (ms_per_step * 1e-3) / 1e9
 
-    # ---- L2-flushed variant: every step timed on its own with a >L2 memset in between
+    # ---- L2-flushed variant: every step timed on its own with a >L2 memset in between (one solve at a time: the
+    # lanes of PG_OPT_LANES are not ordered behind the flush on the timing stream, so they are switched off here)
+    pg.pg_set_option(h, pg.PG_OPT_LANES, 1)
     flush = torch.empty(int(3 * L2_BYTES), dtype=torch.uint8, device="cuda")
     fl = []
     with torch.cuda.stream(st):
@@ -409,7 +416,8 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
-                   "options": "PG_OPT_DENSITY_STABLE (densities resident and complete before the timed loop)",
+                   "options": "PG_OPT_DENSITY_STABLE (densities resident and complete before the timed loop)"
+                              + (", PG_OPT_LANES=2 (independent solves, two in flight; pg_flush before the end event)" if lanes == 2 else ""),
                    "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
                          f"{R * pair_bytes / 1e6:.0f} MB in total vs 126 MB L2"},
         "cells_per_s": value * c.n_r * c.n_phi,
@@ -755,6 +763,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
                     help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")

@@ -19,6 +19,7 @@ PG_ERR_INVALID_ARG, PG_ERR_UNSUPPORTED, PG_ERR_CUDA, PG_ERR_NOMEM, PG_ERR_STATE 
 PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
 PG_NUM_KERNELS = 3
 PG_OPT_DENSITY_STABLE = 1
+PG_OPT_LANES = 2
 PG_SOFT_SYMMETRIC, PG_SOFT_FIELD, PG_SOFT_SOURCE = 0, 1, 2
 KERNEL_NAMES = ("rows_fwd(a2)", "cols(a3+a4r)", "rows_inv(a4phi)")
 
@@ -28,7 +29,7 @@ EXPORTS = (
     "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_set_option", "pg_synchronize",
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
-    "pg_version", "pg_set_softening", "pg_acceleration",
+    "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush",
     "pg3_create", "pg3_set_density", "pg3_potential", "pg3_synchronize", "pg3_destroy", "pg3_launch_count",
     "pg3_algorithmic_bytes", "pg3_last_error",
 )
@@ -65,6 +66,7 @@ def lib():
         L.pg_set_stream.argtypes = [vp, vp]
         L.pg_set_option.argtypes = [vp, i, i]
         L.pg_synchronize.argtypes = [vp]
+        L.pg_flush.argtypes = [vp]
         L.pg_host_alloc.argtypes = [ctypes.POINTER(vp), ctypes.c_size_t]
         L.pg_host_free.argtypes = [vp]
         L.pg_profile.argtypes = [vp, i]
@@ -175,6 +177,10 @@ def pg_set_stream(h, cuda_stream):
 
 def pg_set_option(h, option, value):
     _check(lib().pg_set_option(h, int(option), int(value)), h)
+
+
+def pg_flush(h):
+    _check(lib().pg_flush(h), h)
 
 
 def pg_synchronize(h):
