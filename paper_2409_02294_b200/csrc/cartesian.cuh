@@ -131,7 +131,8 @@ ycols_inv_kernel(const cplx *__restrict__ Yt, cplx *__restrict__ W1, const cplx 
 
 // One-time spectrum of the Green's function: full (unpruned) 2N-point forward transforms along y' then z'.
 //   MODE 0 (y'): column (z', kx) of GW[z'][kx][y'], y' < 2N  ->  GY[(kx M + ey) M + z']                 (complex)
-//   MODE 1 (z'): column (kx, ey) of GY[(kx M + ey) M + z']   ->  Ghat[(kx M + ey) M + ez] = scale Re X  (real: G is even)
+//   MODE 1 (z'): column (kx, ey) of GY[(kx M + ey) M + z']   ->  Ghat[(kx M + ey)][.] = scale Re X      (real: G is even;
+//                stored as its symmetric half in ez, ColShape<N>::KH doubles per column)
 template <int N, int MODE>
 __global__ void __launch_bounds__(ColShape<N>::THREADS)
 gcols_kernel(const cplx *__restrict__ src, cplx *__restrict__ dstc, double *__restrict__ dstr, const cplx *__restrict__ tw,
@@ -167,8 +168,10 @@ gcols_kernel(const cplx *__restrict__ src, cplx *__restrict__ dstc, double *__re
 #pragma unroll
             for (int k = 0; k < 16; ++k) dstc[((long)kx * M + (u + T * k)) * M + zp] = v[k];
         } else {
+            double *kh = dstr + (long)c * (L / 2 + 2);     // symmetric half in ez, the layout cols_kernel reads
 #pragma unroll
-            for (int k = 0; k < 16; ++k) dstr[(long)c * M + (u + T * k)] = scale * v[k].x;
+            for (int k = 0; k < 8; ++k) kh[u + T * k] = scale * v[k].x;
+            if (u == 0) { kh[8 * T] = scale * v[8].x; kh[8 * T + 1] = 0.0; }
         }
     }
 }

@@ -70,7 +70,12 @@ struct ColShape {
     static constexpr int STRIDE = P::LINE;
     static constexpr int THREADS = MODES * T;
     static constexpr size_t LINES = (size_t)MODES * STRIDE * sizeof(cplx);
-    static constexpr size_t STAGE = (size_t)MODES * L * sizeof(double);     // Khat slices of the CTA's modes
+    // Khat is stored as its symmetric half (Khat[k'] = Khat[2N - k'], K is even in the radial lag): KH doubles per
+    // mode -- bins 0..N in the order the threads hold them: entry c T + u is bin  bin0(u) + T c  for c < 8, entry 8 T
+    // is bin N, one more pads the slice to 16 bytes.  Thread u finds its bins c >= 8 in the entries of the thread that
+    // holds bin0 = T - bin0(u) (col_partner), read backwards: half the HBM traffic and half the staging space.
+    static constexpr int KH = L / 2 + 2;
+    static constexpr size_t STAGE = (size_t)MODES * KH * sizeof(double);    // Khat slices of the CTA's modes
     static constexpr size_t SMEM = LINES + STAGE + 16;                      // + one mbarrier
     static constexpr int MIN_CTAS = (THREADS >= 512) ? 1 : (THREADS <= 128 ? 4 : 512 / THREADS);   // cap registers at 128/thread
 };
@@ -421,6 +426,19 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
     }
 }
 
+// thread of a column transform that holds the mirror bins of thread u: bin0(partner) = T - bin0(u)  (u != 0)
+template <int L>
+__device__ __forceinline__ int col_partner(const int u)
+{
+    typedef Plan<L, COL> P;
+    if constexpr (P::NPASS == 3) {
+        const int q = P::T - ((u / P::RB) + P::RA * (u % P::RB));
+        return (q % P::RA) * P::RB + q / P::RA;
+    } else {
+        return P::T - u;
+    }
+}
+
 // ---------------------------------------------------------------- a3 + a4 (r part): columns
 // One CTA owns MODES azimuthal modes; mode m is the column x[0..n_r) = W[m][.].  It is convolved
 // with the Green's kernel over the radial lags, zero-padded to 2 n_r, and cropped back to n_r:
@@ -458,9 +476,10 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     if (tid == 0) {
         const int m0 = blockIdx.x * S::MODES;
         const int nm = (n_modes - m0 < S::MODES) ? n_modes - m0 : S::MODES;
-        bulk_load(kstage, Khat + (long)m0 * L, (unsigned)(nm * L * sizeof(double)), kbar);
+        bulk_load(kstage, Khat + (long)m0 * S::KH, (unsigned)(nm * S::KH * sizeof(double)), kbar);
     }
-    const double *kh = kstage + ml * L;
+    const double *kh = kstage + ml * S::KH;
+    const int kq = (u == 0) ? T : col_partner<L>(u);      // bins c >= 8: entry (15 - c) T + kq
     pdl_wait();                    // W is written by the preceding kernel of the stream
     pdl_launch_dependents();
 
@@ -490,7 +509,7 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     mbar_wait(kbar, 0);
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        const double kv = kh[u + T * k];
+        const double kv = k < 8 ? kh[u + T * k] : kh[kq + T * (15 - k)];
         v[k].x *= kv;
         v[k].y *= kv;
     }
@@ -560,9 +579,10 @@ khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const c
     }
     __syncthreads();
     fwd_c_col<L>(v, line, u);
-    double *kh = Khat + (long)m * L;
+    double *kh = Khat + (long)m * (L / 2 + 2);          // symmetric half, ColShape<NR>::KH doubles per mode
 #pragma unroll
-    for (int k = 0; k < 16; ++k) kh[u + T * k] = scale * v[k].x;
+    for (int k = 0; k < 8; ++k) kh[u + T * k] = scale * v[k].x;
+    if (u == 0) { kh[8 * T] = scale * v[8].x; kh[8 * T + 1] = 0.0; }
 }
 
 // ---------------------------------------------------------------- a5: direct summation
