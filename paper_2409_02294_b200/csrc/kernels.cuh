@@ -299,13 +299,32 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
     Bases<L, ROW> bases;
     bases.load(tw, u, false);
 
+    // Rows carried by whole warps (n_phi >= 1024) are fetched by ONE 1-D bulk asynchronous copy (TMA) per row into a
+    // raw staging row, completion on a per-row mbarrier: the copy engine writes shared memory itself, so the 16
+    // LDGSTS per thread and their LSU issue slots go away.  The next item's row is requested by the row's first thread
+    // right after the row barrier that follows pass A (by then the 64 threads of the row have taken their elements).
+    // Narrower rows keep the per-thread cp.async slots.
+    constexpr bool TMA_IN = (T >= 32) && (P::NPASS == 3) && (ROWS >= 2);
+    constexpr unsigned ROW_BYTES = (HALF ? NPHI / 2 : NPHI) * sizeof(double);
+    cplx *stage_row = smem + ROWS * S::STRIDE + rho * L;
+    unsigned long long *row_bar = reinterpret_cast<unsigned long long *>(smem + ROWS * S::STRIDE + 16 * S::THREADS) + rho;
     auto prefetch = [&](const int item) {
         const int f = item / items_per_field, i = (item % items_per_field) * ROWS + rho;
-        const cplx *x = reinterpret_cast<const cplx *>(sigma + f * sigma_field_stride + (long)i * (HALF ? NPHI / 2 : NPHI)) + u;
+        const double *row = sigma + f * sigma_field_stride + (long)i * (HALF ? NPHI / 2 : NPHI);
+        if constexpr (TMA_IN) {
+            if (u == 0) bulk_load(stage_row, row, ROW_BYTES, row_bar);
+        } else {
+            const cplx *x = reinterpret_cast<const cplx *>(row) + u;
 #pragma unroll
-        for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) cp_async16(stage + jj * S::THREADS, x + T * jj);
-        cp_async_commit();
+            for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) cp_async16(stage + jj * S::THREADS, x + T * jj);
+            cp_async_commit();
+        }
     };
+    if constexpr (TMA_IN) {
+        if (u == 0) mbar_init(row_bar, 1);
+        __syncthreads();
+    }
+    unsigned row_phase = 0;
 
     // Dependence on the preceding kernel of the stream (polargrav.cu decides, `early_load`):
     //   0  Sigma may be its output, and it may still read W: wait before anything else.
@@ -329,10 +348,17 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         cplx v[16];
         const double sc = sc_next;
         sc_next = row_scale(item + gridDim.x);
-        cp_async_wait_all();
+        if constexpr (TMA_IN) {
+            mbar_wait(row_bar, row_phase);
+            row_phase ^= 1;
 #pragma unroll
-        for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage[jj * S::THREADS];
-        if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+            for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage_row[u + T * jj];
+        } else {
+            cp_async_wait_all();
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage[jj * S::THREADS];
+            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        }
         if (rscale != nullptr) {
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) { v[jj].x *= sc; v[jj].y *= sc; }
@@ -341,6 +367,9 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         if constexpr (P::NPASS == 3) {
             const Sync<T, S::THREADS> sync(rho + 1);
             sync();
+            if constexpr (TMA_IN) {
+                if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);   // the row's staging is free
+            }
             fwd_b<L, ROW>(line, bases, u);
         }
         __syncthreads();
