@@ -417,7 +417,7 @@ def run_ours(args):
         "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
                    "options": "PG_OPT_DENSITY_STABLE (densities resident and complete before the timed loop)"
-                              + (", PG_OPT_LANES=2 (independent solves, two in flight; pg_flush before the end event)" if lanes == 2 else ""),
+                              + (f", PG_OPT_LANES={lanes} (independent solves, {lanes} in flight; pg_flush before the end event)" if lanes >= 2 else ""),
                    "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
                          f"{R * pair_bytes / 1e6:.0f} MB in total vs 126 MB L2"},
         "cells_per_s": value * c.n_r * c.n_phi,
@@ -763,7 +763,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
+    ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
                     help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")

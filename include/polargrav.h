@@ -61,6 +61,7 @@ typedef enum {
 
 #define PG_MIN_N 32
 #define PG_MAX_N 2048
+#define PG_MAX_LANES 4 /* PG_OPT_LANES: independent resident solves in flight */
 
 /*
  * pg_create / pg_create_ex -- build a solver for one grid (north_star: pg_create(grid: N_r, N_phi,
@@ -165,16 +166,16 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
  *       entirely alongside the tail of the previous solve's last kernel.  Time series and batches with
  *       densities resident in HBM (the case bench.py times) qualify; a density written by the caller's
  *       kernel enqueued just before does not.
- *   PG_OPT_LANES  (1 or 2, default 1)  Throughput mode for INDEPENDENT resident solves (a batch dealt out one field at a
- *       time, a time series whose steps do not feed each other).  With 2, and PG_OPT_DENSITY_STABLE set, consecutive
- *       PG_MEM_DEVICE pg_potential calls go alternately to two internal streams, so that two solves are in flight and
+ *   PG_OPT_LANES  (1 .. PG_MAX_LANES, default 1)  Throughput mode for INDEPENDENT resident solves (a batch dealt out one field at a
+ *       time, a time series whose steps do not feed each other).  With n >= 2, and PG_OPT_DENSITY_STABLE set, consecutive
+ *       PG_MEM_DEVICE pg_potential calls go in turn to n internal streams, so that n solves are in flight and
  *       the tail and hand-over bubbles of one solve's kernels are filled by the other's.  This CHANGES THE ORDERING
  *       CONTRACT of those calls: their work is not on the solver's stream any more; it is complete after pg_synchronize,
- *       or, stream-ordered, after pg_flush (which makes the solver's stream wait for both lanes).  The caller promises,
+ *       or, stream-ordered, after pg_flush (which makes the solver's stream wait for all lanes).  The caller promises,
  *       for every such call, that the density is complete in memory and that neither the density nor `phi` is read or
  *       written by anything else in flight -- work of the caller or the solve of the call before -- until then.
  *       Host memspaces, pg_profile passes, pg_acceleration and non-symmetric softening keep using the solver's stream.
- *       Setting the option synchronises.  Costs two more pairs of W buffers.
+ *       Setting the option synchronises.  Costs one more pair of W buffers per lane.
  * Returns PG_ERR_INVALID_ARG for an unknown option or value. */
 typedef enum { PG_OPT_DENSITY_STABLE = 1, PG_OPT_LANES = 2 } pg_option;
 pg_status pg_set_option(pg_solver *s, pg_option option, int value);

@@ -21,9 +21,13 @@
 #define PG_ROW_THREADS 128
 #endif
 #ifndef PG_ROW_THREADS_BIG
-#define PG_ROW_THREADS_BIG 128      // n_phi >= 2048: 2 rows per CTA (32-byte runs in W), three CTAs per SM.  (Round 1
-                                    // ran 4 rows / 256 threads / one CTA per SM; since the forward row kernel overlaps the
-                                    // previous solve's tail, three small CTAs hand the SMs over better: 61.4 -> 59.9 us.)
+#define PG_ROW_THREADS_BIG 256      // n_phi >= 2048: 4 rows per CTA (64-byte runs in W), two CTAs per SM.  W is stored
+                                    // transposed, so a CTA of ROWS rows touches it in runs of ROWS * 16 bytes, and the L2
+                                    // serves 32-byte runs at half the rate of 64-byte ones (4.0 against 5.3 (stores) ..
+                                    // 7.7 TB/s (loads), measured): with 2 rows per CTA the row kernels were bound by it.
+#endif
+#ifndef PG_ROW_INLINE_FROM
+#define PG_ROW_INLINE_FROM 2048     // from this n_phi on the row kernels stage their input INSIDE the rows' own lines
 #endif
 
 namespace pgk {
@@ -56,7 +60,12 @@ struct RowShape {
     static constexpr int STRIDE = ((P::LINE + 7) / 8) * 8 + SKEW;   // slots per row line
     static constexpr int THREADS = ROWS * T;
     static constexpr int SLOTS = 17;                                // prefetch slots per thread (16 fwd, 17 inv)
-    static constexpr size_t SMEM = ((size_t)ROWS * STRIDE + (size_t)SLOTS * THREADS) * sizeof(cplx);
+    // INLINE: no staging area of its own -- the next item's input is fetched into the lines themselves once the current
+    // item has left them (a shorter prefetch distance, but half the shared memory: twice the rows resident per SM)
+    static constexpr bool INLINE = (NPHI >= PG_ROW_INLINE_FROM);
+    static_assert(!INLINE || SLOTS * THREADS <= ROWS * STRIDE, "the prefetch slots must fit into the lines");
+    static constexpr size_t SMEM = INLINE ? (size_t)ROWS * STRIDE * sizeof(cplx) + 64
+                                          : ((size_t)ROWS * STRIDE + (size_t)SLOTS * THREADS) * sizeof(cplx);
     // resident CTAs per SM are set by shared memory (227 KB); registers are capped to match
     static constexpr int BY_SMEM = (int)((227 * 1024) / (SMEM + 1024));
     static constexpr int MIN_CTAS = BY_SMEM < 1 ? 1 : (BY_SMEM * THREADS > 512 ? (512 / THREADS > 0 ? 512 / THREADS : 1) : BY_SMEM);
@@ -95,7 +104,15 @@ __device__ __forceinline__ void named_barrier_arrive(const int id, const int thr
 // programmatic dependent launch: wait for the preceding kernel of the stream (no-op without the
 // launch attribute) / allow the following kernel's CTAs to be scheduled as this grid drains
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+#ifndef PG_PDL_EARLY
+#define PG_PDL_EARLY 1              // 0: the dependents are released when a CTA exits (tuning runs)
+#endif
+__device__ __forceinline__ void pdl_launch_dependents()
+{
+#if PG_PDL_EARLY
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
+}
 // orders this thread's view of earlier generic-proxy shared-memory accesses before an asynchronous copy
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -304,15 +321,24 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
     // LDGSTS per thread and their LSU issue slots go away.  The next item's row is requested by the row's first thread
     // right after the row barrier that follows pass A (by then the 64 threads of the row have taken their elements).
     // Narrower rows keep the per-thread cp.async slots.
-    constexpr bool TMA_IN = (T >= 32) && (P::NPASS == 3) && (ROWS >= 2);
+    // INLINE (RowShape): the raw row lands in the row's own line; it is requested once pass C has read the line
+    // (CTA-wide barrier), travels while the split and the transposed stores of the current item run, and a row barrier
+    // between taking the elements and the stores of pass A keeps the two uses of the line apart.
+    constexpr bool INLINE = S::INLINE;
+    static_assert(!INLINE || ((T >= 32) && (P::NPASS == 3)), "inline staging is written for rows carried by whole warps");
+    constexpr bool TMA_IN = INLINE || ((T >= 32) && (P::NPASS == 3) && (ROWS >= 2));
     constexpr unsigned ROW_BYTES = (HALF ? NPHI / 2 : NPHI) * sizeof(double);
-    cplx *stage_row = smem + ROWS * S::STRIDE + rho * L;
-    unsigned long long *row_bar = reinterpret_cast<unsigned long long *>(smem + ROWS * S::STRIDE + 16 * S::THREADS) + rho;
+    cplx *stage_row = INLINE ? line : smem + ROWS * S::STRIDE + rho * L;
+    unsigned long long *row_bar =
+        reinterpret_cast<unsigned long long *>(smem + ROWS * S::STRIDE + (INLINE ? 0 : 16 * S::THREADS)) + rho;
     auto prefetch = [&](const int item) {
         const int f = item / items_per_field, i = (item % items_per_field) * ROWS + rho;
         const double *row = sigma + f * sigma_field_stride + (long)i * (HALF ? NPHI / 2 : NPHI);
         if constexpr (TMA_IN) {
-            if (u == 0) bulk_load(stage_row, row, ROW_BYTES, row_bar);
+            if (u == 0) {
+                if constexpr (INLINE) fence_proxy_async();     // the line was last touched through the generic proxy
+                bulk_load(stage_row, row, ROW_BYTES, row_bar);
+            }
         } else {
             const cplx *x = reinterpret_cast<const cplx *>(row) + u;
 #pragma unroll
@@ -348,11 +374,13 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         cplx v[16];
         const double sc = sc_next;
         sc_next = row_scale(item + gridDim.x);
+        const Sync<T, S::THREADS> sync(rho + 1);
         if constexpr (TMA_IN) {
             mbar_wait(row_bar, row_phase);
             row_phase ^= 1;
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage_row[u + T * jj];
+            if constexpr (INLINE) sync();      // the row's threads have taken their elements: pass A may rewrite the line
         } else {
             cp_async_wait_all();
 #pragma unroll
@@ -365,9 +393,8 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         }
         fwd_a<L, ROW>(v, line, bases, u);
         if constexpr (P::NPASS == 3) {
-            const Sync<T, S::THREADS> sync(rho + 1);
             sync();
-            if constexpr (TMA_IN) {
+            if constexpr (TMA_IN && !INLINE) {
                 if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);   // the row's staging is free
             }
             fwd_b<L, ROW>(line, bases, u);
@@ -375,11 +402,15 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         __syncthreads();
 
         fwd_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
+        if constexpr (INLINE) {
+            __syncthreads();       // every line has been read: the next item's rows may land in them
+            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        }
         cplx *Wf = W + f * w_field_stride + i0 + rp;
         auto store = [&](const int k, const cplx val) { Wf[(long)k * n_rows] = val; };
         if (!special) split_regular<L>(v, un1, q1, store);
         else split_special<L>(v, un1, un2, store);
-        __syncthreads();   // the lines are rewritten by the next item's pass A
+        if constexpr (!INLINE) __syncthreads();   // the lines are rewritten by the next item's pass A
     }
     if (early_load == 2) pdl_wait();
 }
@@ -401,7 +432,10 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
-    cplx *stage = smem + ROWS * S::STRIDE + threadIdx.x;
+    // INLINE (RowShape): the prefetch slots lie inside the lines; the next item's modes are requested once pass A has
+    // taken the current item out of them and travel while pass A computes and the rows are stored
+    constexpr bool INLINE = S::INLINE;
+    cplx *stage = smem + (INLINE ? 0 : ROWS * S::STRIDE) + threadIdx.x;
 
     const int tid = threadIdx.x;
     const int u = tid % T, rho = tid / T;
@@ -438,7 +472,8 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
         cp_async_wait_all();
         if (!special) merge_regular<L>(v, un1, get);
         else merge_special<L>(v, un1, un2, get);
-        if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        if constexpr (INLINE) __syncthreads();     // the slots live in the lines: all of them read before pass C writes
+        else if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
         inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
         __syncthreads();
 
@@ -447,11 +482,16 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
             inv_b<L, ROW>(line, bases, u);
             sync();
         }
-        inv_a<L, ROW>(v, line, bases, u);
+        inv_a_load<L, ROW>(v, line, u);
+        if constexpr (INLINE) {
+            __syncthreads();       // the lines are free: the next item's modes may land in them
+            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        }
+        inv_a_compute<L, ROW>(v, bases, u);
         cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * (HALF ? NPHI / 2 : NPHI));
 #pragma unroll
         for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
-        __syncthreads();   // the lines are rewritten by the next item's pass C
+        if constexpr (!INLINE) __syncthreads();   // the lines are rewritten by the next item's pass C
     }
 }
 

@@ -51,11 +51,11 @@ struct pg_solver {
     // PG_OPT_LANES: consecutive resident solves alternate between two internal streams (each with its own pair of W
     // buffers), so that the tail and the hand-over bubbles of one solve's kernels are filled by the other's
     int lanes = 1, lane_next = 0;
-    cudaStream_t lane_stream[2] = {nullptr, nullptr};
-    cudaEvent_t lane_done[2] = {nullptr, nullptr};
-    cplx *lane_W[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
-    int lane_w_next[2] = {0, 0};
-    bool lane_used[2] = {false, false};
+    cudaStream_t lane_stream[PG_MAX_LANES] = {};
+    cudaEvent_t lane_done[PG_MAX_LANES] = {};
+    cplx *lane_W[PG_MAX_LANES][2] = {};
+    int lane_w_next[PG_MAX_LANES] = {};
+    bool lane_used[PG_MAX_LANES] = {};
     double *d_khat = nullptr;     // [half+1][2][n_r]
     cplx *d_tw_row = nullptr;     // Plan<n_phi/2, ROW> twiddle table
     cplx *d_tw_col = nullptr;     // Plan<2 n_r, COL> twiddle table
@@ -589,19 +589,25 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         double *out = d_phi;
         return solve_variant(s, d_sigma, d_W, batch, 1, &kind, &out);
     }
-    if (s->lanes == 2 && s->density_stable && !s->sigma_from_host && !ev && d_W == s->d_W) {
+    if (s->lanes >= 2 && s->density_stable && !s->sigma_from_host && !ev && d_W == s->d_W) {
         // two solves in flight: this one goes to the lane the previous one did not take.  The caller has promised
         // (polargrav.h, PG_OPT_LANES) that density and potential are touched by nothing else in flight.
         const int L = s->lane_next;
-        s->lane_next ^= 1;
+        s->lane_next = (L + 1) % s->lanes;
         cudaStream_t lst = s->lane_stream[L];
         cplx *W = s->lane_W[L][s->lane_w_next[L]];
         s->lane_w_next[L] ^= 1;
         const int early = overlaps_early_release_output(s->device, lst, d_sigma, (size_t)batch * s->field * sizeof(double)) ? 0 : 2;
-        pg_status st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early);
-        if (st != PG_OK) return st;
+        pg_status st = PG_OK;
+#ifdef PG_KERNEL_MASK          // tuning runs: a subset of the three kernels (results are then meaningless)
+        if ((PG_KERNEL_MASK & 1) && (st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early)) != PG_OK) return st;
+        if ((PG_KERNEL_MASK & 2) && (st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
+        if ((PG_KERNEL_MASK & 4) && (st = rows_inv(s, W, d_phi, batch, ws, fs, lst)) != PG_OK) return st;
+#else
+        if ((st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early)) != PG_OK) return st;
         if ((st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
         if ((st = rows_inv(s, W, d_phi, batch, ws, fs, lst)) != PG_OK) return st;
+#endif
         PG_CUDA(s, cudaEventRecord(s->lane_done[L], lst));
         s->lane_used[L] = true;
         return PG_OK;
@@ -680,10 +686,10 @@ pg_status launch_direct(pg_solver *s, const double *d_sigma, double *d_phi, int 
     return PG_OK;
 }
 
-pg_status lanes_enable(pg_solver *s)
+pg_status lanes_enable(pg_solver *s, int n_lanes)
 {
     const size_t w_bytes = (size_t)s->max_batch * (s->half + 1) * s->n_r * sizeof(cplx);
-    for (int L = 0; L < 2; ++L) {
+    for (int L = 0; L < n_lanes; ++L) {
         if (!s->lane_stream[L]) PG_CUDA(s, cudaStreamCreateWithFlags(&s->lane_stream[L], cudaStreamNonBlocking));
         if (!s->lane_done[L]) PG_CUDA(s, cudaEventCreateWithFlags(&s->lane_done[L], cudaEventDisableTiming));
         for (int k = 0; k < 2; ++k)
@@ -694,7 +700,7 @@ pg_status lanes_enable(pg_solver *s)
 // everything the lanes have in flight is complete when this returns
 pg_status lanes_drain(pg_solver *s)
 {
-    for (int L = 0; L < 2; ++L)
+    for (int L = 0; L < PG_MAX_LANES; ++L)
         if (s->lane_stream[L]) {
             PG_CUDA(s, cudaStreamSynchronize(s->lane_stream[L]));
             forget_early_release_output(s->device, s->lane_stream[L]);
@@ -706,7 +712,7 @@ pg_status lanes_drain(pg_solver *s)
 void free_all(pg_solver *s)
 {
     if (!s) return;
-    for (int L = 0; L < 2; ++L) {
+    for (int L = 0; L < PG_MAX_LANES; ++L) {
         if (s->lane_stream[L]) { cudaStreamSynchronize(s->lane_stream[L]); forget_early_release_output(s->device, s->lane_stream[L]); cudaStreamDestroy(s->lane_stream[L]); }
         if (s->lane_done[L]) cudaEventDestroy(s->lane_done[L]);
         for (int k = 0; k < 2; ++k) cudaFree(s->lane_W[L][k]);
@@ -1114,13 +1120,14 @@ pg_status pg_set_option(pg_solver *s, pg_option option, int value)
     switch (option) {
         case PG_OPT_DENSITY_STABLE: s->density_stable = value != 0; return PG_OK;
         case PG_OPT_LANES: {
-            if (value != 1 && value != 2) { set_err(s, "PG_OPT_LANES: 1 or 2"); return PG_ERR_INVALID_ARG; }
+            if (value < 1 || value > PG_MAX_LANES) { set_err(s, "PG_OPT_LANES: 1 .. %d", PG_MAX_LANES); return PG_ERR_INVALID_ARG; }
             DeviceGuard guard(s->device);
             PG_CUDA(s, cudaStreamSynchronize(s->stream));      // what is in flight on the solver's stream comes first
             pg_status st = lanes_drain(s);
             if (st != PG_OK) return st;
-            if (value == 2 && (st = lanes_enable(s)) != PG_OK) return st;
+            if (value >= 2 && (st = lanes_enable(s, value)) != PG_OK) return st;
             s->lanes = value;
+            s->lane_next = 0;
             return PG_OK;
         }
     }
@@ -1132,7 +1139,7 @@ pg_status pg_flush(pg_solver *s)
 {
     if (!s) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
-    for (int L = 0; L < 2; ++L)
+    for (int L = 0; L < PG_MAX_LANES; ++L)
         if (s->lane_used[L]) PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->lane_done[L], 0));
     return PG_OK;
 }
