@@ -272,7 +272,7 @@ def test_fed_back_potential_with_another_solver_in_between():
 
 @pytest.mark.parametrize("n_r,n_phi,batch", [(1024, 1024, 2), (2048, 2048, 1), (256, 512, 3)])
 def test_two_lanes_equal_one_lane_bit_for_bit(n_r, n_phi, batch):
-    """PG_OPT_LANES = 2: independent resident solves alternate between two internal streams; results are those of the
+    """PG_OPT_LANES = 2, 3: independent resident solves go in turn to that many internal streams; results are those of the
     ordinary path bit for bit, complete after pg_flush + a sync of the solver's stream (or pg_synchronize)."""
     st = torch.cuda.Stream()
     s = pg.Solver(n_r, n_phi, 1.0, 1000.0, 0.01, max_batch=batch, device=0, cuda_stream=st.cuda_stream)
@@ -295,15 +295,16 @@ def test_two_lanes_equal_one_lane_bit_for_bit(n_r, n_phi, batch):
             return [o.cpu().numpy() for o in out]
 
         one = run(1)
-        two = run(2)
-        for a, b in zip(one, two):
-            assert np.array_equal(a, b) and (a < 0).all()
+        for lanes in (2, 3):
+            many = run(lanes)
+            for a, b in zip(one, many):
+                assert np.array_equal(a, b) and (a < 0).all()
         # a host-staged solve in between keeps working (it uses the solver's own stream)
         host = s.potential_host(sig[0].cpu().numpy())
         assert np.array_equal(host, one[0])
         pg.pg_set_option(s.h, pg.PG_OPT_LANES, 1)
         with pytest.raises(pg.PolargravError) as e:
-            pg.pg_set_option(s.h, pg.PG_OPT_LANES, 3)
+            pg.pg_set_option(s.h, pg.PG_OPT_LANES, 5)          # PG_MAX_LANES = 4
         assert e.value.status == pg.PG_ERR_INVALID_ARG
     finally:
         s.close()
