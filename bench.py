@@ -275,8 +275,14 @@ def run_ours(args):
     pg.pg_set_option(h, pg.PG_OPT_DENSITY_STABLE, 1)
     # the solves of the timed loop are independent (distinct resident buffer pairs): two in flight (PG_OPT_LANES),
     # joined into the timing stream by pg_flush before the end event.  Off for the host-bound small grids.
-    lanes = args.lanes if args.lanes else (2 if c.n_r * c.n_phi >= 1 << 20 else 1)
+    # Grids of up to 512 x 512 take the fused single-launch path (PG_OPT_FUSED, on by default) and are bound by the
+    # host's launch rate: four lanes keep four of those launches in flight.
+    small = c.n_r <= 512 and c.n_phi <= 512
+    lanes = args.lanes if args.lanes else (2 if c.n_r * c.n_phi >= 1 << 20 else (4 if small else 1))
     pg.pg_set_option(h, pg.PG_OPT_LANES, lanes)
+    if args.no_fused:
+        pg.pg_set_option(h, pg.PG_OPT_FUSED, 0)
+    fused = small and not args.no_fused
     r, phi, _ = solver.grid()
     n_fields = R * c.batch
     distinct = min(n_fields, 8 if c.n_r * c.n_phi >= 1 << 22 else 32)
@@ -416,6 +422,8 @@ def run_ours(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
+                   "path": ("one cooperative launch per solve (fused_solve_kernel: a2 | grid barrier | a3+a4r | grid barrier | a4phi)"
+                            if fused else "three launches per solve (rows_fwd, cols, rows_inv) chained by programmatic dependent launch"),
                    "options": "PG_OPT_DENSITY_STABLE (densities resident and complete before the timed loop)"
                               + (f", PG_OPT_LANES={lanes} (independent solves, {lanes} in flight; pg_flush before the end event)" if lanes >= 2 else ""),
                    "l2": f"inputs larger than L2: steps rotate over {R} distinct (Sigma,Phi) buffer pairs, "
@@ -453,6 +461,8 @@ def run_ours(args):
     for a in pin_in + pin_out:
         a.free()
     solver.close()
+    if small and rank == 0:
+        line["batched"] = batched_small(cfg, st, args)
     if world > 1:
         import torch.distributed as dist
         dist.barrier()
@@ -463,6 +473,46 @@ def run_ours(args):
         sys.stderr.write(f"bench.py: PARITY GATE FAILED: {parity}; the timing above does not count\n")
         return 3
     return 0
+
+
+def batched_small(cfg, st, args):
+    """Configs 1-3 are single solves and bound by the host's launch rate.  The same C-ABI calls take a batch: 32
+    independent fields per pg_set_density / pg_potential pair, one launch set for all of them."""
+    import torch
+    from paper_2409_02294_b200 import binding as pg
+    c = CONFIGS[cfg]
+    B = 32
+    s = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, max_batch=B, device=torch.cuda.current_device(), cuda_stream=st.cuda_stream)
+    try:
+        pg.pg_set_option(s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        if args.no_fused:
+            pg.pg_set_option(s.h, pg.PG_OPT_FUSED, 0)
+        r, phi, _ = s.grid()
+        base = np.stack([make_sigma(cfg, r, phi, b % 4) for b in range(B)])
+        R = int(min(16, max(2, -(-4 * L2_BYTES // (2 * base.nbytes)))))
+        d_sig = [torch.from_numpy(np.roll(base, 7 * p, axis=2)).cuda() for p in range(R)]
+        d_phi = [torch.empty_like(x) for x in d_sig]
+        torch.cuda.synchronize()
+        steps = max(args.steps, 20)
+        ms = []
+        n0 = pg.pg_launch_count(s.h)
+        for rep in range(REPEATS + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(st)
+            for k in range(steps):
+                pg.pg_set_density(s.h, d_sig[k % R], B, pg.PG_MEM_DEVICE)
+                pg.pg_potential(s.h, d_phi[k % R], B, pg.PG_MEM_DEVICE)
+            e1.record(st)
+            torch.cuda.synchronize()
+            if rep:
+                ms.append(e0.elapsed_time(e1) / steps)
+        launches = (pg.pg_launch_count(s.h) - n0) / ((REPEATS + 1) * steps)
+        med = float(np.median(ms))
+        return {"batch": B, "ms_per_batch": med, "solves_per_s": B * 1e3 / med, "launches_per_batch": launches,
+                "what": f"{B} independent fields per pg_set_density / pg_potential pair (resident), median of {REPEATS} repeats of {steps} batches"}
+    finally:
+        s.close()
 
 
 FP64_LANES_PER_CLK_PER_SM = 64
@@ -764,6 +814,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
+    ap.add_argument("--no-fused", action="store_true", help="small grids: force the three-kernel path (PG_OPT_FUSED = 0)")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
                     help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")

@@ -176,8 +176,13 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
  *       written by anything else in flight -- work of the caller or the solve of the call before -- until then.
  *       Host memspaces, pg_profile passes, pg_acceleration and non-symmetric softening keep using the solver's stream.
  *       Setting the option synchronises.  Costs one more pair of W buffers per lane.
+ *   PG_OPT_FUSED  (0 or 1, default 1)  Grids of 64 .. 512 cells per axis are solved by ONE cooperative kernel launch
+ *       (the three steps a2, a3+a4r, a4phi separated by grid-wide barriers, the spectrum staying in the L2) instead of
+ *       three launches, as long as the batch is small enough for all its CTAs to be resident at once: such solves are
+ *       bound by the host's launch rate, not by the GPU.  Same arithmetic, bit-identical results.  0 forces the
+ *       three-kernel path (which pg_profile passes, pg_acceleration and non-symmetric softening always take).
  * Returns PG_ERR_INVALID_ARG for an unknown option or value. */
-typedef enum { PG_OPT_DENSITY_STABLE = 1, PG_OPT_LANES = 2 } pg_option;
+typedef enum { PG_OPT_DENSITY_STABLE = 1, PG_OPT_LANES = 2, PG_OPT_FUSED = 3 } pg_option;
 pg_status pg_set_option(pg_solver *s, pg_option option, int value);
 /* Stream-ordered join of the lanes of PG_OPT_LANES: work enqueued on the solver's stream after this call runs after
  * every solve enqueued before it.  No-op with one lane.  Returns after enqueue. */

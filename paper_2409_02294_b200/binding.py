@@ -20,6 +20,7 @@ PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
 PG_NUM_KERNELS = 3
 PG_OPT_DENSITY_STABLE = 1
 PG_OPT_LANES = 2
+PG_OPT_FUSED = 3
 PG_SOFT_SYMMETRIC, PG_SOFT_FIELD, PG_SOFT_SOURCE = 0, 1, 2
 KERNEL_NAMES = ("rows_fwd(a2)", "cols(a3+a4r)", "rows_inv(a4phi)")
 

@@ -274,11 +274,23 @@ template <int RC>
 __host__ __device__ constexpr int pad(int p) { return p + p / RC; }
 
 // ------------------------------------------------------------------ barriers
-// Sync<T, CTA>: barrier among the T threads of one transform.  When a transform is made of whole
+// Barrier among ALL threads that run a kernel body.  CtaBarrier: the whole CTA (the stand-alone kernels).
+// PartBarrier<N>: the first N threads of a larger CTA, on named barrier 15 (the fused small-grid kernel, kernels.cuh,
+// whose phases use different thread counts; N is a multiple of 32).
+struct CtaBarrier {
+    static __device__ __forceinline__ void sync() { __syncthreads(); }
+};
+template <int N>
+struct PartBarrier {
+    static_assert(N % 32 == 0, "whole warps");
+    static __device__ __forceinline__ void sync() { asm volatile("bar.sync 15, %0;" ::"n"(N) : "memory"); }
+};
+
+// Sync<T, CTA, CB>: barrier among the T threads of one transform.  When a transform is made of whole
 // warps (T >= 32) and the CTA holds several transforms, each gets its own named barrier
-// (bar.sync id, T), so that the transforms of a CTA drift apart instead of marching in lockstep;
-// otherwise the CTA-wide barrier is used (every thread of the CTA then runs the same sequence).
-template <int T, int CTA_THREADS>
+// (bar.sync id, T; ids 1 .. 8), so that the transforms of a CTA drift apart instead of marching in lockstep;
+// otherwise the barrier CB of all the body's threads is used (every thread then runs the same sequence).
+template <int T, int CTA_THREADS, class CB = CtaBarrier>
 struct Sync {
     static constexpr bool NAMED = (T >= 32) && (T < CTA_THREADS);
     int id;
@@ -286,7 +298,7 @@ struct Sync {
     __device__ __forceinline__ void operator()() const
     {
         if constexpr (NAMED) asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(T) : "memory");
-        else __syncthreads();
+        else CB::sync();
     }
 };
 

@@ -15,6 +15,7 @@
 //                                         (entry c T + u is bin  bin0(u) + T c); all normalisations folded in
 //   tw_row, tw_col : compact twiddle tables (Plan<L,KIND>::TW_*), long double on the host
 #pragma once
+#include <cooperative_groups.h>
 #include "fft.cuh"
 
 #ifndef PG_ROW_THREADS
@@ -289,16 +290,17 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // round trip.
 // HALF (the x pass of the 3-D mesh path, cartesian.cuh): the rows in memory hold only the first n_phi/2 reals, the
 // second half of the transform's input is zero padding that is never read.
-template <int NPHI, bool HALF = false>
-__global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
-rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
-                const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
-                const long w_field_stride, const int early_load)
+// The body runs as CTA `block` of `nblocks` (block / nblocks in the stand-alone kernel; the fused small-grid kernel
+// passes its own) on the shared memory it is given; CB is the barrier among the body's threads.
+template <int NPHI, bool HALF, class CB>
+__device__ __forceinline__ void rows_fwd_body(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
+                                              const double *__restrict__ rscale, const int n_rows, const int n_items,
+                                              const long sigma_field_stride, const long w_field_stride, const int early_load,
+                                              const int block, const int nblocks, unsigned char *smem_raw)
 {
     typedef RowShape<NPHI> S;
     typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     cplx *stage = smem + ROWS * S::STRIDE + threadIdx.x;
 
@@ -348,7 +350,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
     };
     if constexpr (TMA_IN) {
         if (u == 0) mbar_init(row_bar, 1);
-        __syncthreads();
+        CB::sync();
     }
     unsigned row_phase = 0;
 
@@ -360,7 +362,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
     //      two): this kernel depends on nothing that runs before it.  It does all its work at once --
     //      filling the SMs the preceding kernel leaves idle in its last, uneven round -- and waits at its
     //      END, so that its own completion still implies that of everything before it.
-    int item = blockIdx.x;
+    int item = block;
     if (early_load && item < n_items) prefetch(item);
     if (early_load < 2) pdl_wait();
     pdl_launch_dependents();
@@ -369,12 +371,12 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         return (rscale != nullptr && it < n_items) ? __ldg(&rscale[(it % items_per_field) * ROWS + rho]) : 1.0;
     };
     double sc_next = row_scale(item);
-    for (; item < n_items; item += gridDim.x) {
+    for (; item < n_items; item += nblocks) {
         const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
         cplx v[16];
         const double sc = sc_next;
-        sc_next = row_scale(item + gridDim.x);
-        const Sync<T, S::THREADS> sync(rho + 1);
+        sc_next = row_scale(item + nblocks);
+        const Sync<T, S::THREADS, CB> sync(rho + 1);
         if constexpr (TMA_IN) {
             mbar_wait(row_bar, row_phase);
             row_phase ^= 1;
@@ -385,7 +387,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
             cp_async_wait_all();
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) v[jj] = (HALF && jj >= 8) ? make_double2(0.0, 0.0) : stage[jj * S::THREADS];
-            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+            if (item + nblocks < n_items) prefetch(item + nblocks);
         }
         if (rscale != nullptr) {
 #pragma unroll
@@ -395,24 +397,34 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
         if constexpr (P::NPASS == 3) {
             sync();
             if constexpr (TMA_IN && !INLINE) {
-                if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);   // the row's staging is free
+                if (item + nblocks < n_items) prefetch(item + nblocks);   // the row's staging is free
             }
             fwd_b<L, ROW>(line, bases, u);
         }
-        __syncthreads();
+        CB::sync();
 
         fwd_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
         if constexpr (INLINE) {
-            __syncthreads();       // every line has been read: the next item's rows may land in them
-            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+            CB::sync();       // every line has been read: the next item's rows may land in them
+            if (item + nblocks < n_items) prefetch(item + nblocks);
         }
         cplx *Wf = W + f * w_field_stride + i0 + rp;
         auto store = [&](const int k, const cplx val) { Wf[(long)k * n_rows] = val; };
         if (!special) split_regular<L>(v, un1, q1, store);
         else split_special<L>(v, un1, un2, store);
-        if constexpr (!INLINE) __syncthreads();   // the lines are rewritten by the next item's pass A
+        if constexpr (!INLINE) CB::sync();   // the lines are rewritten by the next item's pass A
     }
     if (early_load == 2) pdl_wait();
+}
+template <int NPHI, bool HALF = false>
+__global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
+rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cplx *__restrict__ tw,
+                const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
+                const long w_field_stride, const int early_load)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    rows_fwd_body<NPHI, HALF, CtaBarrier>(sigma, W, tw, rscale, n_rows, n_items, sigma_field_stride, w_field_stride, early_load,
+                                          blockIdx.x, gridDim.x, smem_raw);
 }
 
 // ---------------------------------------------------------------- a4 (phi part): rows inverse
@@ -421,16 +433,15 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
 // row, inverse pass C; the remaining passes with u fastest; multiplies row i by oscale_i
 // (= r_i^{-1/2}) and stores Phi_i.
 // HALF: only the first n_phi/2 reals of every output row are stored, in rows of that length (the crop of the x pass).
-template <int NPHI, bool HALF = false>
-__global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
-rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
-                const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
-                const long phi_field_stride)
+template <int NPHI, bool HALF, class CB>
+__device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
+                                              const double *__restrict__ oscale, const int n_rows, const int n_items,
+                                              const long w_field_stride, const long phi_field_stride, const int block,
+                                              const int nblocks, unsigned char *smem_raw)
 {
     typedef RowShape<NPHI> S;
     typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     // INLINE (RowShape): the prefetch slots lie inside the lines; the next item's modes are requested once pass A has
     // taken the current item out of them and travel while pass A computes and the rows are stored
@@ -463,36 +474,46 @@ rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx
 
     pdl_wait();                    // W is written by the preceding kernel of the stream
     pdl_launch_dependents();
-    int item = blockIdx.x;
+    int item = block;
     if (item < n_items) prefetch(item);
-    for (; item < n_items; item += gridDim.x) {
+    for (; item < n_items; item += nblocks) {
         const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
         cplx v[16];
         const double sc = __ldg(&oscale[i0 + rho]);
         cp_async_wait_all();
         if (!special) merge_regular<L>(v, un1, get);
         else merge_special<L>(v, un1, un2, get);
-        if constexpr (INLINE) __syncthreads();     // the slots live in the lines: all of them read before pass C writes
-        else if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+        if constexpr (INLINE) CB::sync();     // the slots live in the lines: all of them read before pass C writes
+        else if (item + nblocks < n_items) prefetch(item + nblocks);
         inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
-        __syncthreads();
+        CB::sync();
 
         if constexpr (P::NPASS == 3) {
-            const Sync<T, S::THREADS> sync(rho + 1);
+            const Sync<T, S::THREADS, CB> sync(rho + 1);
             inv_b<L, ROW>(line, bases, u);
             sync();
         }
         inv_a_load<L, ROW>(v, line, u);
         if constexpr (INLINE) {
-            __syncthreads();       // the lines are free: the next item's modes may land in them
-            if (item + (int)gridDim.x < n_items) prefetch(item + gridDim.x);
+            CB::sync();       // the lines are free: the next item's modes may land in them
+            if (item + nblocks < n_items) prefetch(item + nblocks);
         }
         inv_a_compute<L, ROW>(v, bases, u);
         cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * (HALF ? NPHI / 2 : NPHI));
 #pragma unroll
         for (int jj = 0; jj < (HALF ? 8 : 16); ++jj) y[u + T * jj] = make_double2(v[jj].x * sc, v[jj].y * sc);
-        if constexpr (!INLINE) __syncthreads();   // the lines are rewritten by the next item's pass C
+        if constexpr (!INLINE) CB::sync();   // the lines are rewritten by the next item's pass C
     }
+}
+template <int NPHI, bool HALF = false>
+__global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
+rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
+                const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
+                const long phi_field_stride)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    rows_inv_body<NPHI, HALF, CtaBarrier>(W, phi, tw, oscale, n_rows, n_items, w_field_stride, phi_field_stride, blockIdx.x,
+                                          gridDim.x, smem_raw);
 }
 
 // thread of a column transform that holds the mirror bins of thread u: bin0(partner) = T - bin0(u)  (u != 0)
@@ -517,33 +538,33 @@ __device__ __forceinline__ int col_partner(const int u)
 // radix-RA DFT, fft.cuh dft_zero_upper) and writes only 8 (the crop: the last inverse pass keeps the
 // lower half of its outputs, idft_lower_half).  The padded array and the discarded half are never
 // formed in memory (a3: multiply fused into the last forward pass; a4: inverse with fused crop).
-template <int NR>
-__global__ void __launch_bounds__(ColShape<NR>::THREADS, ColShape<NR>::MIN_CTAS)
-cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw, const int n_modes,
-            const long w_field_stride)
+// The body transforms mode group `group` of field `field` (group / field in the stand-alone kernel).
+template <int NR, class CB>
+__device__ __forceinline__ void cols_body(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw,
+                                          const int n_modes, const long w_field_stride, const int group, const int field,
+                                          unsigned char *smem_raw)
 {
     typedef ColShape<NR> S;
     typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
 
     const int tid = threadIdx.x;
     const int u = tid % T, ml = tid / T;
-    const int m_raw = blockIdx.x * S::MODES + ml;
+    const int m_raw = group * S::MODES + ml;
     const bool live = m_raw < n_modes;
     const int mode = live ? m_raw : n_modes - 1;
     cplx *line = smem + ml * S::STRIDE;
-    cplx *col = W + blockIdx.y * w_field_stride + (long)mode * NR;
+    cplx *col = W + field * w_field_stride + (long)mode * NR;
 
     // the Khat slices of this CTA's modes are contiguous: one bulk asynchronous copy into shared
     // memory, issued now and waited for after the forward transform
     double *kstage = reinterpret_cast<double *>(smem_raw + S::LINES);
     unsigned long long *kbar = reinterpret_cast<unsigned long long *>(smem_raw + S::LINES + S::STAGE);
     if (tid == 0) mbar_init(kbar, 1);
-    __syncthreads();
+    CB::sync();
     if (tid == 0) {
-        const int m0 = blockIdx.x * S::MODES;
+        const int m0 = group * S::MODES;
         const int nm = (n_modes - m0 < S::MODES) ? n_modes - m0 : S::MODES;
         bulk_load(kstage, Khat + (long)m0 * S::KH, (unsigned)(nm * S::KH * sizeof(double)), kbar);
     }
@@ -558,7 +579,7 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
     Bases<L, COL> bases;
     bases.load(tw, u, false);
 
-    const Sync<T, S::THREADS> sync(ml + 1);
+    const Sync<T, S::THREADS, CB> sync(ml + 1);
     fwd_a_compute_zero_upper<L, COL>(v, bases, u);
     fwd_a_store<L, COL>(v, line, u);
     // Three-pass plans: pass B (in place) and pass C of a thread touch only slots of the 16 blocks
@@ -595,6 +616,59 @@ cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *_
 #pragma unroll
         for (int jj = 0; jj < 8; ++jj) col[u + T * jj] = v[jj];
     }
+}
+template <int NR>
+__global__ void __launch_bounds__(ColShape<NR>::THREADS, ColShape<NR>::MIN_CTAS)
+cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw, const int n_modes,
+            const long w_field_stride)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cols_body<NR, CtaBarrier>(W, Khat, tw, n_modes, w_field_stride, blockIdx.x, blockIdx.y, smem_raw);
+}
+
+// ---------------------------------------------------------------- small grids: the whole solve in ONE launch
+// For grids of up to 512 x 512 the three kernels above take 1-3 us each and a solve is bound by the host's launch rate
+// (three launches, 7-14 us).  fused_solve_kernel runs the three bodies in one COOPERATIVE launch, separated by
+// grid-wide barriers; W stays in the L2 in between.  Phase a2 / a4phi: CTA b takes the row items b, b + gridDim.x, ...
+// with its first RowShape::THREADS threads; phase a3+a4r: CTA b takes mode group b (field b / groups) with its first
+// ColShape::THREADS threads.  The host sizes the grid to max(items, groups * batch) and uses this kernel only when that
+// many CTAs are resident at once (polargrav.cu, solve_fields).
+template <int NR, int NPHI>
+struct FusedShape {
+    typedef RowShape<NPHI> RS;
+    typedef ColShape<NR> CS;
+    static_assert(!RS::INLINE && NPHI >= 64 && NPHI <= 512 && NR >= 64 && NR <= 512, "fused path: 64 .. 512 per axis");
+    static constexpr int THREADS = RS::THREADS > CS::THREADS ? RS::THREADS : CS::THREADS;
+    static constexpr size_t SMEM = RS::SMEM > CS::SMEM ? RS::SMEM : CS::SMEM;
+};
+template <int NR, int NPHI>
+__global__ void __launch_bounds__(FusedShape<NR, NPHI>::THREADS)
+fused_solve_kernel(const double *__restrict__ sigma, double *__restrict__ phi, cplx *__restrict__ W,
+                   const double *__restrict__ Khat, const cplx *__restrict__ tw_row, const cplx *__restrict__ tw_col,
+                   const double *__restrict__ rscale, const double *__restrict__ oscale, const int batch,
+                   const long field_stride, const long w_field_stride)
+{
+    typedef FusedShape<NR, NPHI> F;
+    typedef typename F::RS RS;
+    typedef typename F::CS CS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const int n_items = (NR / RS::ROWS) * batch;
+    constexpr int n_modes = NPHI / 2 + 1;
+    constexpr int groups = (n_modes + CS::MODES - 1) / CS::MODES;
+
+    if (threadIdx.x < RS::THREADS)
+        rows_fwd_body<NPHI, false, PartBarrier<RS::THREADS>>(sigma, W, tw_row, rscale, NR, n_items, field_stride,
+                                                            w_field_stride, 0, blockIdx.x, gridDim.x, smem_raw);
+    grid.sync();
+    fence_proxy_async();           // the Khat slices arrive by bulk copy in shared memory the row phase has used
+    if ((int)blockIdx.x < groups * batch && threadIdx.x < CS::THREADS)
+        cols_body<NR, PartBarrier<CS::THREADS>>(W, Khat, tw_col, n_modes, w_field_stride, blockIdx.x % groups,
+                                                blockIdx.x / groups, smem_raw);
+    grid.sync();
+    if (threadIdx.x < RS::THREADS)
+        rows_inv_body<NPHI, false, PartBarrier<RS::THREADS>>(W, phi, tw_row, oscale, NR, n_items, w_field_stride,
+                                                            field_stride, blockIdx.x, gridDim.x, smem_raw);
 }
 
 // ---------------------------------------------------------------- a1: Green's kernel

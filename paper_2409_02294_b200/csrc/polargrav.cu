@@ -35,6 +35,10 @@ struct pg_solver {
     int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
     int sm_count = 0, row_ctas = 0;   // persistent grid of the row kernels
+    // small grids (64 .. 512 per axis): the whole solve in one cooperative launch (kernels.cuh, fused_solve_kernel)
+    int fused = 1;                    // PG_OPT_FUSED
+    int fused_cap = 0;                // CTAs of the fused kernel resident at once (0: the grid has no fused kernel)
+    int fused_items = 0, fused_groups = 0;   // row items and mode groups per field
     int half = 0;      // H = n_phi/2: azimuthal modes are 0..H (H + 1 columns of W)
     size_t field = 0;  // n_r * n_phi
 
@@ -290,6 +294,76 @@ pg_status launch_cols(pg_solver *s, cplx *Z, int batch, long z_stride, cudaStrea
                           (const cplx *)s->d_tw_col, modes, z_stride));
     s->launches++;
     return PG_OK;
+}
+
+// ---- small grids: one cooperative launch per solve
+template <int NR, int NPHI>
+pg_status prepare_fused(pg_solver *s)
+{
+    typedef pgk::FusedShape<NR, NPHI> F;
+    PG_CUDA(s, cudaFuncSetAttribute(pgk::fused_solve_kernel<NR, NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F::SMEM));
+    int occ = 0;
+    PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pgk::fused_solve_kernel<NR, NPHI>, F::THREADS, F::SMEM));
+    s->fused_cap = occ * s->sm_count;
+    s->fused_items = NR / F::RS::ROWS;
+    s->fused_groups = (NPHI / 2 + 1 + F::CS::MODES - 1) / F::CS::MODES;
+    return PG_OK;
+}
+template <int NR, int NPHI>
+pg_status launch_fused(pg_solver *s, const double *sigma, double *phi, cplx *W, int batch, cudaStream_t st)
+{
+    typedef pgk::FusedShape<NR, NPHI> F;
+    const int items = s->fused_items * batch, cols = s->fused_groups * batch;
+    const int grid = items > cols ? items : cols;
+    long fs = (long)s->field, ws = (long)(s->half + 1) * s->n_r;
+    const double *khat = s->d_khat, *rs_in = s->d_rs_in, *rs_out = s->d_rs_out;
+    const cplx *tw_row = s->d_tw_row, *tw_col = s->d_tw_col;
+    void *args[] = {(void *)&sigma, (void *)&phi, (void *)&W, (void *)&khat, (void *)&tw_row, (void *)&tw_col,
+                    (void *)&rs_in, (void *)&rs_out, (void *)&batch, (void *)&fs, (void *)&ws};
+    PG_CUDA(s, cudaLaunchCooperativeKernel((const void *)pgk::fused_solve_kernel<NR, NPHI>, dim3(grid), dim3(F::THREADS), args,
+                                           F::SMEM, st));
+    s->launches++;
+    return PG_OK;
+}
+#define PG_FUSED_DISPATCH_PHI(NR, CALL)                         \
+    switch (s->n_phi) {                                         \
+        case 64: return CALL(NR, 64);                           \
+        case 128: return CALL(NR, 128);                         \
+        case 256: return CALL(NR, 256);                         \
+        case 512: return CALL(NR, 512);                         \
+        default: return PG_ERR_UNSUPPORTED;                     \
+    }
+#define PG_FUSED_DISPATCH(CALL)                                 \
+    switch (s->n_r) {                                           \
+        case 64: PG_FUSED_DISPATCH_PHI(64, CALL)                \
+        case 128: PG_FUSED_DISPATCH_PHI(128, CALL)              \
+        case 256: PG_FUSED_DISPATCH_PHI(256, CALL)              \
+        case 512: PG_FUSED_DISPATCH_PHI(512, CALL)              \
+        default: return PG_ERR_UNSUPPORTED;                     \
+    }
+bool fused_size(const pg_solver *s)
+{
+    return s->n_r >= 64 && s->n_r <= 512 && s->n_phi >= 64 && s->n_phi <= 512;
+}
+pg_status prepare_kernels_fused(pg_solver *s)
+{
+    if (!fused_size(s)) return PG_OK;
+#define CALL(NR, NPHI) prepare_fused<NR, NPHI>(s)
+    PG_FUSED_DISPATCH(CALL)
+#undef CALL
+}
+pg_status fused_solve(pg_solver *s, const double *sigma, double *phi, cplx *W, int batch, cudaStream_t st)
+{
+#define CALL(NR, NPHI) launch_fused<NR, NPHI>(s, sigma, phi, W, batch, st)
+    PG_FUSED_DISPATCH(CALL)
+#undef CALL
+}
+// the fused kernel serves this solve: enabled, symmetric softening, no per-kernel profiling, all its CTAs resident at once
+bool fused_ok(const pg_solver *s, int batch, bool profiled)
+{
+    if (!s->fused || s->fused_cap <= 0 || profiled) return false;
+    const int items = s->fused_items * batch, cols = s->fused_groups * batch;
+    return (items > cols ? items : cols) <= s->fused_cap;
 }
 
 template <int NR>
@@ -597,8 +671,13 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         cudaStream_t lst = s->lane_stream[L];
         cplx *W = s->lane_W[L][s->lane_w_next[L]];
         s->lane_w_next[L] ^= 1;
-        const int early = overlaps_early_release_output(s->device, lst, d_sigma, (size_t)batch * s->field * sizeof(double)) ? 0 : 2;
         pg_status st = PG_OK;
+        if (fused_ok(s, batch, false)) {
+            if ((st = fused_solve(s, d_sigma, d_phi, W, batch, lst)) != PG_OK) return st;
+            s->lane_used[L] = true;        // joined by pg_flush / pg_synchronize
+            return PG_OK;
+        }
+        const int early = overlaps_early_release_output(s->device, lst, d_sigma, (size_t)batch * s->field * sizeof(double)) ? 0 : 2;
 #ifdef PG_KERNEL_MASK          // tuning runs: a subset of the three kernels (results are then meaningless)
         if ((PG_KERNEL_MASK & 1) && (st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early)) != PG_OK) return st;
         if ((PG_KERNEL_MASK & 2) && (st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
@@ -608,9 +687,12 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         if ((st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
         if ((st = rows_inv(s, W, d_phi, batch, ws, fs, lst)) != PG_OK) return st;
 #endif
-        PG_CUDA(s, cudaEventRecord(s->lane_done[L], lst));
-        s->lane_used[L] = true;
+        s->lane_used[L] = true;            // joined by pg_flush / pg_synchronize
         return PG_OK;
+    }
+    if (fused_ok(s, batch, ev != nullptr)) {
+        s->last_w = d_W;
+        return fused_solve(s, d_sigma, d_phi, d_W, batch, s->stream);
     }
     // How much rows_fwd depends on the kernel before it (kernels.cuh): with a stable density that does not
     // alias the potential still being written, the first item is fetched early (1); if the solve also
@@ -819,6 +901,7 @@ pg_status create_impl(pg_solver *s)
 
     if ((st = prepare_kernels_rows(s)) != PG_OK) return st;
     if ((st = prepare_kernels_cols(s)) != PG_OK) return st;
+    if ((st = prepare_kernels_fused(s)) != PG_OK) return st;
     return build_khat(s);
 }
 
@@ -1119,6 +1202,7 @@ pg_status pg_set_option(pg_solver *s, pg_option option, int value)
     if (!s) return PG_ERR_INVALID_ARG;
     switch (option) {
         case PG_OPT_DENSITY_STABLE: s->density_stable = value != 0; return PG_OK;
+        case PG_OPT_FUSED: s->fused = value != 0; return PG_OK;
         case PG_OPT_LANES: {
             if (value < 1 || value > PG_MAX_LANES) { set_err(s, "PG_OPT_LANES: 1 .. %d", PG_MAX_LANES); return PG_ERR_INVALID_ARG; }
             DeviceGuard guard(s->device);
@@ -1140,7 +1224,10 @@ pg_status pg_flush(pg_solver *s)
     if (!s) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
     for (int L = 0; L < PG_MAX_LANES; ++L)
-        if (s->lane_used[L]) PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->lane_done[L], 0));
+        if (s->lane_used[L]) {
+            PG_CUDA(s, cudaEventRecord(s->lane_done[L], s->lane_stream[L]));
+            PG_CUDA(s, cudaStreamWaitEvent(s->stream, s->lane_done[L], 0));
+        }
     return PG_OK;
 }
 

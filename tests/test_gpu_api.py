@@ -308,3 +308,69 @@ def test_two_lanes_equal_one_lane_bit_for_bit(n_r, n_phi, batch):
         assert e.value.status == pg.PG_ERR_INVALID_ARG
     finally:
         s.close()
+
+
+@pytest.mark.parametrize("n_r,n_phi,batch", [(64, 64, 1), (64, 64, 5), (256, 256, 1), (512, 512, 1), (512, 512, 3),
+                                             (64, 512, 2), (512, 64, 2), (128, 256, 4)])
+def test_fused_single_launch_equals_three_kernels_bit_for_bit(n_r, n_phi, batch):
+    """PG_OPT_FUSED (default on): grids of 64 .. 512 cells per axis are solved by ONE cooperative launch (the three
+    kernel bodies separated by grid-wide barriers) as long as all its CTAs are resident at once; larger batches fall
+    back to the three kernels.  Same arithmetic: bit-identical potentials, one launch per solve instead of three, and
+    parity with the oracle on field 0."""
+    st = torch.cuda.Stream()
+    s = pg.Solver(n_r, n_phi, 1.0, 300.0, 0.01, max_batch=batch, device=0, cuda_stream=st.cuda_stream)
+    try:
+        sig = np.stack([random_sigma(n_r, n_phi, 4000 + b) for b in range(batch)])
+        d_s = torch.from_numpy(sig).cuda()
+        got = {}
+        for fused in (0, 1):
+            pg.pg_set_option(s.h, pg.PG_OPT_FUSED, fused)
+            out = torch.zeros_like(d_s)
+            n0 = pg.pg_launch_count(s.h)
+            for _ in range(3):                                   # back to back: the W workspace is reused safely
+                pg.pg_set_density(s.h, d_s, batch, pg.PG_MEM_DEVICE)
+                pg.pg_potential(s.h, out, batch, pg.PG_MEM_DEVICE)
+            pg.pg_synchronize(s.h)
+            got[fused] = (out.cpu().numpy(), pg.pg_launch_count(s.h) - n0)
+        assert np.array_equal(got[0][0], got[1][0])
+        assert got[0][1] == 9
+        assert got[1][1] in (3, 9)                               # 9: the batch does not fit one resident grid
+        if batch == 1 or n_r * n_phi <= 128 * 256:
+            assert got[1][1] == 3
+        ref = oracle.potential_o1(n_r, n_phi, 1.0, 300.0, 0.01, sig[0])
+        assert np.linalg.norm(got[1][0][0] - ref) / np.linalg.norm(ref) <= 1e-10
+        assert np.abs(got[1][0][0] / ref - 1).max() <= 1e-9
+        # the host-staged path goes through the same fused launch, one field at a time
+        host = s.potential_host(sig)
+        assert np.array_equal(host, got[1][0])
+    finally:
+        s.close()
+
+
+def test_fused_solves_on_four_lanes_equal_the_ordinary_path():
+    """Small grids in throughput mode: PG_OPT_LANES = 4 deals the fused launches out over four internal streams."""
+    n_r = n_phi = 256
+    st = torch.cuda.Stream()
+    s = pg.Solver(n_r, n_phi, 1.0, 500.0, 0.01, device=0, cuda_stream=st.cuda_stream)
+    try:
+        pg.pg_set_option(s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        K = 9
+        sig = [torch.from_numpy(random_sigma(n_r, n_phi, 5000 + k)[None]).cuda() for k in range(K)]
+        torch.cuda.synchronize()
+        res = {}
+        for lanes, fused in ((1, 0), (4, 1)):
+            pg.pg_set_option(s.h, pg.PG_OPT_LANES, lanes)
+            pg.pg_set_option(s.h, pg.PG_OPT_FUSED, fused)
+            out = [torch.zeros_like(x) for x in sig]
+            torch.cuda.synchronize()
+            for rep in range(3):
+                for k in range(K):
+                    pg.pg_set_density(s.h, sig[k], 1, pg.PG_MEM_DEVICE)
+                    pg.pg_potential(s.h, out[k], 1, pg.PG_MEM_DEVICE)
+            pg.pg_flush(s.h)
+            st.synchronize()
+            res[lanes] = [o.cpu().numpy() for o in out]
+        for a, b in zip(res[1], res[4]):
+            assert np.array_equal(a, b) and (a < 0).all()
+    finally:
+        s.close()
