@@ -9,3 +9,4 @@ from .polar_oracle import (  # noqa: F401
     cart_potential, cart_potential_targets, cart_self_constant,
 )
 from .definition_numpy import potential_definition_numpy  # noqa: F401
+from . import nested_oracle  # noqa: F401  (NEXT-3: nested meshes, step-by-step algorithm)
