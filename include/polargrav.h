@@ -230,7 +230,7 @@ const char *pg_version(void);
  *                     copied to an owned device buffer (PG_MEM_HOST blocks until `rho` may be reused).
  *   pg3_potential     PG_MEM_DEVICE / PG_MEM_HOST_PINNED return after enqueue; PG_MEM_HOST blocks until filled.
  *                     `phi` may not overlap a device density.  PG_ERR_STATE before any pg3_set_density.
- * Nested levels and their exchange across GPUs (Fig. 8) are NEXT-3 and not built. */
+ * Nested levels and their exchange across GPUs (Fig. 8) are the pg3n_* calls below. */
 typedef struct pg3_solver pg3_solver; /* opaque */
 pg_status pg3_create(pg3_solver **out, int n, double box, int device, void *cuda_stream);
 pg_status pg3_set_density(pg3_solver *s, const double *rho, pg_memspace where);
@@ -240,6 +240,44 @@ pg_status pg3_destroy(pg3_solver *s); /* pg3_destroy(NULL) is a no-op returning 
 long pg3_launch_count(const pg3_solver *s);
 double pg3_algorithmic_bytes(const pg3_solver *s);
 const char *pg3_last_error(const pg3_solver *s); /* s may be NULL: last error of a failed pg3_create */
+
+/* ---------------------------------------------------------------- nested 3-D mesh levels
+ * The paper's distributed scheme: depth D nested meshes of n^3 cells with a common centre, each half the edge of the
+ * one before, "each nested mesh ... allocated one GPU" (Fig. 8 :306).  PAPER.md prints no coupling
+ * scheme (it is in ref. [13], :376, not available); readings N1-N6 of DESIGN.md section 3:
+ *   N1  box_l = box0 / 2^l; level l+1 covers the central (n/2)^3 cells [n/4, 3n/4)^3 of level l, 2 cells per parent cell.
+ *   N2  restriction, finest first: the central (n/2)^3 cells of rho_l are replaced by the means of their 8 children.
+ *   N3  own_l = Phi[rho_l] and, for l < D-1, out_l = Phi[rho_l with the central cells zeroed], each the isolated
+ *       single-level convolution pg3_potential computes (readings C1-C4).
+ *   N4  E_0 = 0, E_(l+1) = P[out_l + E_l]: the potential of everything outside box_(l+1).
+ *   N5  P: trilinear interpolation between the parent's cell centres onto the child's (weights 3/4, 1/4); the parent
+ *       cells [n/4 - 1, 3n/4]^3 -- (n/2 + 2)^3 values -- cross the level boundary.
+ *   N6  Phi_l = own_l + E_l.
+ * One pg3n_level per level; all calls enqueue on the level's (borrowed) stream and return, except PG_MEM_HOST
+ * copies, which block.  The two messages between neighbouring levels are plain device arrays the CALLER moves: by
+ * pointer when both levels live on one GPU, by NCCL send / recv (NVLink) when each level has its own GPU
+ * (paper_2409_02294_b200/nested.py does either).  Call order for one solve:
+ *   pg3n_set_density on every level                          (copied: N2 rewrites the centre)
+ *   l = D-1 .. 1:  pg3n_restrict(l, msg) ; pg3n_absorb(l-1, msg)              msg: (n/2)^3 doubles, device
+ *   every level:   pg3n_solve                                                  (independent across levels)
+ *   l = 0 .. D-1:  pg3n_add_exterior(l, l ? halo : NULL) ; if l < D-1: pg3n_pack_exterior(l, halo)
+ *                                                                              halo: (n/2 + 2)^3 doubles, device
+ *   pg3n_potential on every level.
+ * n in {32, 64, 128, 256}; device pointers 16-byte aligned.  PG_ERR_STATE for calls out of order or on the wrong end
+ * of the hierarchy (restrict on level 0, absorb / pack on the finest level). */
+typedef struct pg3n_level pg3n_level; /* opaque */
+pg_status pg3n_create(pg3n_level **out, int n, double box0, int level, int depth, int device, void *cuda_stream);
+pg_status pg3n_set_density(pg3n_level *s, const double *rho, pg_memspace where);
+pg_status pg3n_restrict(pg3n_level *s, double *child_mean_out);
+pg_status pg3n_absorb(pg3n_level *s, const double *child_mean);
+pg_status pg3n_solve(pg3n_level *s);
+pg_status pg3n_add_exterior(pg3n_level *s, const double *parent_halo);
+pg_status pg3n_pack_exterior(pg3n_level *s, double *halo_out);
+pg_status pg3n_potential(pg3n_level *s, double *phi, pg_memspace where);
+pg_status pg3n_synchronize(pg3n_level *s);
+pg_status pg3n_destroy(pg3n_level *s); /* pg3n_destroy(NULL) is a no-op returning PG_OK */
+long pg3n_launch_count(const pg3n_level *s);
+const char *pg3n_last_error(const pg3n_level *s); /* s may be NULL: last error of a failed pg3n_create */
 
 #ifdef __cplusplus
 }

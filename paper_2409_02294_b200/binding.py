@@ -33,6 +33,8 @@ EXPORTS = (
     "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush",
     "pg3_create", "pg3_set_density", "pg3_potential", "pg3_synchronize", "pg3_destroy", "pg3_launch_count",
     "pg3_algorithmic_bytes", "pg3_last_error",
+    "pg3n_create", "pg3n_set_density", "pg3n_restrict", "pg3n_absorb", "pg3n_solve", "pg3n_add_exterior",
+    "pg3n_pack_exterior", "pg3n_potential", "pg3n_synchronize", "pg3n_destroy", "pg3n_launch_count", "pg3n_last_error",
 )
 
 _lib = None
@@ -77,8 +79,20 @@ def lib():
         L.pg3_potential.argtypes = [vp, vp, i]
         L.pg3_synchronize.argtypes = [vp]
         L.pg3_destroy.argtypes = [vp]
+        L.pg3n_create.argtypes = [ctypes.POINTER(vp), i, d, i, i, i, vp]
+        L.pg3n_set_density.argtypes = [vp, vp, i]
+        L.pg3n_restrict.argtypes = [vp, vp]
+        L.pg3n_absorb.argtypes = [vp, vp]
+        L.pg3n_solve.argtypes = [vp]
+        L.pg3n_add_exterior.argtypes = [vp, vp]
+        L.pg3n_pack_exterior.argtypes = [vp, vp]
+        L.pg3n_potential.argtypes = [vp, vp, i]
+        L.pg3n_synchronize.argtypes = [vp]
+        L.pg3n_destroy.argtypes = [vp]
         for name in EXPORTS:
             getattr(L, name).restype = i
+        L.pg3n_launch_count.argtypes = [vp]; L.pg3n_launch_count.restype = l
+        L.pg3n_last_error.argtypes = [vp]; L.pg3n_last_error.restype = ctypes.c_char_p
         L.pg3_launch_count.argtypes = [vp]; L.pg3_launch_count.restype = l
         L.pg3_algorithmic_bytes.argtypes = [vp]; L.pg3_algorithmic_bytes.restype = d
         L.pg3_last_error.argtypes = [vp]; L.pg3_last_error.restype = ctypes.c_char_p
@@ -260,6 +274,64 @@ def pg3_algorithmic_bytes(h):
 
 def pg3_last_error(h=None):
     return lib().pg3_last_error(h).decode()
+
+
+# ------------------------------------------------------------------ NEXT-3: nested 3-D mesh levels
+def _check3n(st, handle=None):
+    if st != PG_OK:
+        msg = lib().pg3n_last_error(handle).decode()
+        raise PolargravError(st, f"{status_string(st)}: {msg}")
+
+
+def pg3n_create(n, box0, level, depth, device=-1, cuda_stream=None):
+    h = ctypes.c_void_p()
+    _check3n(lib().pg3n_create(ctypes.byref(h), n, box0, level, depth, device,
+                               ctypes.c_void_p(cuda_stream) if cuda_stream else None))
+    return h
+
+
+def pg3n_set_density(h, rho, where):
+    _check3n(lib().pg3n_set_density(h, _ptr(rho), where), h)
+
+
+def pg3n_restrict(h, child_mean_out):
+    _check3n(lib().pg3n_restrict(h, _ptr(child_mean_out)), h)
+
+
+def pg3n_absorb(h, child_mean):
+    _check3n(lib().pg3n_absorb(h, _ptr(child_mean)), h)
+
+
+def pg3n_solve(h):
+    _check3n(lib().pg3n_solve(h), h)
+
+
+def pg3n_add_exterior(h, parent_halo):
+    _check3n(lib().pg3n_add_exterior(h, _ptr(parent_halo)), h)
+
+
+def pg3n_pack_exterior(h, halo_out):
+    _check3n(lib().pg3n_pack_exterior(h, _ptr(halo_out)), h)
+
+
+def pg3n_potential(h, phi, where):
+    _check3n(lib().pg3n_potential(h, _ptr(phi), where), h)
+
+
+def pg3n_synchronize(h):
+    _check3n(lib().pg3n_synchronize(h), h)
+
+
+def pg3n_destroy(h):
+    _check3n(lib().pg3n_destroy(h))
+
+
+def pg3n_launch_count(h):
+    return int(lib().pg3n_launch_count(h))
+
+
+def pg3n_last_error(h=None):
+    return lib().pg3n_last_error(h).decode()
 
 
 # ------------------------------------------------------------------ convenience wrapper

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpolargrav.so")
 SOURCES = [os.path.join(CSRC, "polargrav.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fft.cuh", "kernels.cuh", "variants.cuh", "cartesian.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fft.cuh", "kernels.cuh", "variants.cuh", "cartesian.cuh", "nested.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "polargrav.h")]
 
 NVCC_FLAGS = [

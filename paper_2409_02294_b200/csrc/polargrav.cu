@@ -8,6 +8,7 @@
 #include "kernels.cuh"
 #include "variants.cuh"
 #include "cartesian.cuh"
+#include "nested.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -1591,5 +1592,224 @@ double pg3_algorithmic_bytes(const pg3_solver *s)
     const double w1 = 16.0 * (n + 1) * n * n, yt = 16.0 * (n + 1) * 2.0 * n * n, gh = 8.0 * (n + 1) * 4.0 * n * n;
     return 2.0 * 8.0 * cells + 2.0 * w1 + 2.0 * w1 + 4.0 * yt + gh;
 }
+
+}  // extern "C"
+
+// =================================================================== NEXT-3: nested 3-D mesh levels
+// One object per level ("each nested mesh was allocated one GPU"): the level's own single-level solver
+// (box_0 / 2^level) plus the buffers of the coupling steps of nested.cuh.  Every call enqueues on the level's stream
+// and returns; the caller (paper_2409_02294_b200/nested.py) moves the two small boundary messages between levels --
+// (n/2)^3 restricted densities upwards, (n/2 + 2)^3 exterior potentials downwards -- by pointer on one GPU or by
+// NCCL send / recv between GPUs.
+struct pg3n_level {
+    int n = 0, level = 0, depth = 1, device = 0;
+    pg3_solver *mesh = nullptr;
+    double *d_rho = nullptr, *d_mask = nullptr, *d_own = nullptr, *d_out = nullptr, *d_ext = nullptr, *d_phi = nullptr;
+    bool have_rho = false, solved = false, have_phi = false;
+    long launches = 0;
+    char err[512] = "";
+};
+
+namespace {
+
+void set_err3n(pg3n_level *s, const char *fmt, ...)
+{
+    char *dst = s ? s->err : g_create_error;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+}
+#define PG3N_CUDA(s, call)                                                                     \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            set_err3n((s), "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return e_ == cudaErrorMemoryAllocation ? PG_ERR_NOMEM : PG_ERR_CUDA;               \
+        }                                                                                      \
+    } while (0)
+
+unsigned blocks_for(long count) { return (unsigned)((count + 255) / 256); }
+
+bool dev_ptr_ok(pg3n_level *s, const void *p, const char *what)
+{
+    if (!p) { set_err3n(s, "%s is NULL", what); return false; }
+    if (((uintptr_t)p & 15u) != 0) { set_err3n(s, "%s must be a 16-byte aligned device pointer", what); return false; }
+    return true;
+}
+
+void nest_free(pg3n_level *s)
+{
+    if (!s) return;
+    cudaFree(s->d_rho); cudaFree(s->d_mask); cudaFree(s->d_own); cudaFree(s->d_out); cudaFree(s->d_ext); cudaFree(s->d_phi);
+    if (s->mesh) pg3_destroy(s->mesh);
+    delete s;
+}
+
+}  // namespace
+
+extern "C" {
+
+pg_status pg3n_create(pg3n_level **out, int n, double box0, int level, int depth, int device, void *cuda_stream)
+{
+    g_create_error[0] = 0;
+    if (!out) { set_err3n(nullptr, "out is NULL"); return PG_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (!(box0 > 0.0) || !std::isfinite(box0) || depth < 1 || depth > 32 || level < 0 || level >= depth) {
+        set_err3n(nullptr, "invalid argument: need box0 > 0, 1 <= depth <= 32, 0 <= level < depth");
+        return PG_ERR_INVALID_ARG;
+    }
+    pg3n_level *s = new (std::nothrow) pg3n_level;
+    if (!s) { set_err3n(nullptr, "out of host memory"); return PG_ERR_NOMEM; }
+    s->n = n; s->level = level; s->depth = depth;
+    pg_status rc = pg3_create(&s->mesh, n, std::ldexp(box0, -level), device, cuda_stream);   // N1: box_l = box_0 / 2^l
+    if (rc != PG_OK) { delete s; return rc; }
+    s->device = s->mesh->device;
+    DeviceGuard guard(s->device);
+    const size_t bytes = (size_t)n * n * n * sizeof(double);
+    double **bufs[] = {&s->d_rho, &s->d_mask, &s->d_own, &s->d_out, &s->d_ext, &s->d_phi};
+    for (double **b : bufs) {
+        if (b == &s->d_mask || b == &s->d_out) { if (level == depth - 1) continue; }          // the finest level has no child
+        if (cudaMalloc((void **)b, bytes) != cudaSuccess) {
+            set_err3n(nullptr, "out of device memory for the level's buffers");
+            nest_free(s);
+            return PG_ERR_NOMEM;
+        }
+    }
+    *out = s;
+    return PG_OK;
+}
+
+pg_status pg3n_set_density(pg3n_level *s, const double *rho, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!rho) { set_err3n(s, "pg3n_set_density: rho is NULL"); return PG_ERR_INVALID_ARG; }
+    if (where != PG_MEM_DEVICE && where != PG_MEM_HOST && where != PG_MEM_HOST_PINNED) {
+        set_err3n(s, "pg3n_set_density: unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(s->device);
+    cudaStream_t st = s->mesh->inner->stream;
+    const size_t bytes = (size_t)s->n * s->n * s->n * sizeof(double);
+    // always copied: N2 rewrites the central cells of every level that has a child
+    PG3N_CUDA(s, cudaMemcpyAsync(s->d_rho, rho, bytes, where == PG_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    if (where == PG_MEM_HOST) PG3N_CUDA(s, cudaStreamSynchronize(st));
+    s->have_rho = true; s->solved = false; s->have_phi = false;
+    return PG_OK;
+}
+
+pg_status pg3n_restrict(pg3n_level *s, double *child_mean_out)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
+    if (s->level == 0) { set_err3n(s, "level 0 has no parent to restrict to"); return PG_ERR_STATE; }
+    if (!dev_ptr_ok(s, child_mean_out, "child_mean_out")) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
+    const long q = s->n / 2;
+    pgk::nest_restrict_kernel<<<blocks_for(q * q * q), 256, 0, s->mesh->inner->stream>>>(s->d_rho, child_mean_out, s->n);
+    PG3N_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+pg_status pg3n_absorb(pg3n_level *s, const double *child_mean)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
+    if (s->level == s->depth - 1) { set_err3n(s, "the finest level has no child to absorb"); return PG_ERR_STATE; }
+    if (!dev_ptr_ok(s, child_mean, "child_mean")) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
+    const long q = s->n / 2;
+    pgk::nest_absorb_kernel<<<blocks_for(q * q * q), 256, 0, s->mesh->inner->stream>>>(s->d_rho, child_mean, s->n);
+    PG3N_CUDA(s, cudaGetLastError());
+    s->launches++;
+    s->solved = false;
+    return PG_OK;
+}
+
+pg_status pg3n_solve(pg3n_level *s)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
+    DeviceGuard guard(s->device);
+    const long before = s->mesh->inner->launches;
+    pg_status rc = cart_run(s->mesh, s->d_rho, s->d_own);                                  // N3: own_l
+    if (rc == PG_OK && s->level < s->depth - 1) {
+        const long cells = (long)s->n * s->n * s->n;
+        pgk::nest_mask_kernel<<<blocks_for(cells), 256, 0, s->mesh->inner->stream>>>(s->d_rho, s->d_mask, s->n);
+        s->launches++;
+        rc = cart_run(s->mesh, s->d_mask, s->d_out);                                       // N3: out_l
+    }
+    if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", s->mesh->err); return rc; }
+    PG3N_CUDA(s, cudaGetLastError());
+    s->launches += s->mesh->inner->launches - before;
+    s->solved = true; s->have_phi = false;
+    return PG_OK;
+}
+
+pg_status pg3n_add_exterior(pg3n_level *s, const double *parent_halo)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!s->solved) { set_err3n(s, "pg3n_add_exterior before pg3n_solve"); return PG_ERR_STATE; }
+    if (s->level == 0 && parent_halo) { set_err3n(s, "level 0 is isolated: parent_halo must be NULL"); return PG_ERR_INVALID_ARG; }
+    if (s->level > 0 && !dev_ptr_ok(s, parent_halo, "parent_halo")) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
+    const long cells = (long)s->n * s->n * s->n;
+    pgk::nest_prolong_kernel<<<blocks_for(cells), 256, 0, s->mesh->inner->stream>>>(parent_halo, s->d_own, s->d_ext, s->d_phi, s->n);
+    PG3N_CUDA(s, cudaGetLastError());
+    s->launches++;
+    s->have_phi = true;
+    return PG_OK;
+}
+
+pg_status pg3n_pack_exterior(pg3n_level *s, double *halo_out)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!s->have_phi) { set_err3n(s, "pg3n_pack_exterior before pg3n_add_exterior"); return PG_ERR_STATE; }
+    if (s->level == s->depth - 1) { set_err3n(s, "the finest level has no child"); return PG_ERR_STATE; }
+    if (!dev_ptr_ok(s, halo_out, "halo_out")) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
+    const long m = s->n / 2 + 2;
+    pgk::nest_pack_kernel<<<blocks_for(m * m * m), 256, 0, s->mesh->inner->stream>>>(s->d_out, s->d_ext, halo_out, s->n);
+    PG3N_CUDA(s, cudaGetLastError());
+    s->launches++;
+    return PG_OK;
+}
+
+pg_status pg3n_potential(pg3n_level *s, double *phi, pg_memspace where)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!phi) { set_err3n(s, "pg3n_potential: phi is NULL"); return PG_ERR_INVALID_ARG; }
+    if (!s->have_phi) { set_err3n(s, "pg3n_potential before pg3n_add_exterior"); return PG_ERR_STATE; }
+    if (where != PG_MEM_DEVICE && where != PG_MEM_HOST && where != PG_MEM_HOST_PINNED) {
+        set_err3n(s, "unknown memspace %d", (int)where);
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(s->device);
+    cudaStream_t st = s->mesh->inner->stream;
+    const size_t bytes = (size_t)s->n * s->n * s->n * sizeof(double);
+    PG3N_CUDA(s, cudaMemcpyAsync(phi, s->d_phi, bytes, where == PG_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (where == PG_MEM_HOST) PG3N_CUDA(s, cudaStreamSynchronize(st));
+    return PG_OK;
+}
+
+pg_status pg3n_synchronize(pg3n_level *s)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    return pg3_synchronize(s->mesh);
+}
+
+pg_status pg3n_destroy(pg3n_level *s)
+{
+    if (!s) return PG_OK;
+    DeviceGuard guard(s->device);
+    cudaStreamSynchronize(s->mesh->inner->stream);
+    nest_free(s);
+    return PG_OK;
+}
+
+long pg3n_launch_count(const pg3n_level *s) { return s ? s->launches : 0; }
+
+const char *pg3n_last_error(const pg3n_level *s) { return s ? s->err : g_create_error; }
 
 }  // extern "C"

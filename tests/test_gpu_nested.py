@@ -1,0 +1,100 @@
+"""Parity of the nested-mesh path (row NEXT-3 of SURVEY.md 8(f): Fig. 8 :306; readings N1-N6)
+against oracle/nested_oracle.py, element by element on seeded densities, level by level, and of each coupling kernel
+against its oracle step.  Bar: rel-L2 <= 1e-10, max pointwise relative <= 1e-9."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import nested_oracle as no
+from paper_2409_02294_b200 import binding as pg
+from paper_2409_02294_b200 import nested
+
+pytestmark = pytest.mark.gpu
+
+
+def level_rho(n, level, seed):
+    """A centrally condensed clump sampled on the level's cells plus seeded clumps and 1 % noise; non-negative."""
+    rng = np.random.Generator(np.random.PCG64(2409022940 + 7000 * n + 10 * seed + level))
+    x = (np.arange(n) + 0.5 - n / 2.0) / n / 2.0**level
+    z, y, xx = np.meshgrid(x, x, x, indexing="ij")
+    rho = 1.0 / (1.0 + (xx**2 + y**2 + z**2) / 0.05**2)
+    for _ in range(4):
+        c = rng.uniform(-0.4, 0.4, 3) / 2.0**level
+        w = rng.uniform(0.03, 0.1) / 2.0**level
+        rho += rng.uniform(0.5, 2.0) * np.exp(-((xx - c[0]) ** 2 + (y - c[1]) ** 2 + (z - c[2]) ** 2) / (2 * w * w))
+    return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))
+
+
+def check(got, ref, what):
+    l2 = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.abs(got / ref - 1.0).max()
+    assert l2 <= 1e-10 and mx <= 1e-9, f"{what}: rel-L2 {l2:.3e}, max rel {mx:.3e}"
+
+
+@pytest.mark.parametrize("n,depth", [(32, 1), (32, 2), (32, 3), (64, 2)])
+def test_nested_levels_on_one_gpu_vs_oracle(n, depth):
+    box0 = 8.0
+    rhos = [level_rho(n, l, depth) for l in range(depth)]
+    ref, _ = no.nested_potential(n, box0, rhos)
+    np_ = nested.NestedPotential(n, box0, depth, device=0)
+    try:
+        d_rho = {l: torch.from_numpy(rhos[l]).cuda() for l in range(depth)}
+        d_out = {l: torch.empty_like(d_rho[l]) for l in range(depth)}
+        for rep in range(2):                                   # twice: the message buffers are reused safely
+            np_.solve(d_rho, d_out)
+        np_.synchronize()
+        for l in range(depth):
+            got = d_out[l].cpu().numpy()
+            assert (got < 0).all()
+            check(got, ref[l], f"n={n} depth={depth} level {l}")
+        assert np_.launches() > 0
+    finally:
+        np_.close()
+
+
+def test_coupling_kernels_step_by_step_and_call_order_errors():
+    n, box0 = 32, 4.0
+    rng = np.random.default_rng(11)
+    coarse, fine = rng.random((n, n, n)), rng.random((n, n, n))
+    st = torch.cuda.current_stream().cuda_stream
+    h0 = pg.pg3n_create(n, box0, 0, 2, 0, st)
+    h1 = pg.pg3n_create(n, box0, 1, 2, 0, st)
+    try:
+        n_mean, n_halo = nested.message_counts(n)
+        mean = torch.zeros(n_mean, dtype=torch.float64, device="cuda")
+        halo = torch.zeros(n_halo, dtype=torch.float64, device="cuda")
+        with pytest.raises(pg.PolargravError) as e:            # nothing set yet
+            pg.pg3n_restrict(h1, mean)
+        assert e.value.status == pg.PG_ERR_STATE
+        pg.pg3n_set_density(h0, coarse, pg.PG_MEM_HOST)
+        pg.pg3n_set_density(h1, torch.from_numpy(fine).cuda(), pg.PG_MEM_DEVICE)
+        for bad in (lambda: pg.pg3n_restrict(h0, mean), lambda: pg.pg3n_absorb(h1, mean),
+                    lambda: pg.pg3n_add_exterior(h0, None), lambda: pg.pg3n_pack_exterior(h0, halo)):
+            with pytest.raises(pg.PolargravError) as e:
+                bad()
+            assert e.value.status == pg.PG_ERR_STATE
+        pg.pg3n_restrict(h1, mean)
+        pg.pg3n_synchronize(h1)
+        assert np.array_equal(mean.cpu().numpy().reshape(n // 2, n // 2, n // 2), no.restrict(fine))      # N2, same order
+        pg.pg3n_absorb(h0, mean)
+        pg.pg3n_solve(h0); pg.pg3n_solve(h1)
+        pg.pg3n_add_exterior(h0, None)
+        pg.pg3n_pack_exterior(h0, halo)
+        with pytest.raises(pg.PolargravError) as e:            # level 1 needs its parent's values
+            pg.pg3n_add_exterior(h1, None)
+        assert e.value.status == pg.PG_ERR_INVALID_ARG
+        pg.pg3n_add_exterior(h1, halo)
+        out0 = np.empty((n, n, n)); out1 = np.empty((n, n, n))
+        pg.pg3n_potential(h0, out0, pg.PG_MEM_HOST); pg.pg3n_potential(h1, out1, pg.PG_MEM_HOST)
+        ref, rho = no.nested_potential(n, box0, [coarse, fine])
+        check(out0, ref[0], "level 0"); check(out1, ref[1], "level 1")
+        # the packed message is (out_0 + E_0) on the parent cells that cross the boundary; E_1 is its prolongation
+        import oracle
+        ref_halo = no.pack_halo(oracle.cart_potential(n, box0, no.mask_centre(rho[0])))
+        got_halo = halo.cpu().numpy().reshape((n // 2 + 2,) * 3)
+        check(got_halo, ref_halo, "halo")
+        ext1 = out1 - oracle.cart_potential(n, box0 / 2, fine)
+        assert np.abs(ext1 - no.prolong(got_halo, n)).max() <= 1e-11 * np.abs(out1).max()
+    finally:
+        pg.pg3n_destroy(h0); pg.pg3n_destroy(h1)
