@@ -678,6 +678,124 @@ def make_rho3(n: int, seed: int):
     return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))
 
 
+def run_nested(args):
+    """--nested D [--cart N]: the paper's distributed scheme (row NEXT-3): D nested mesh levels of N^3 cells
+    (Fig. 8 :306; readings N1-N6).  One process: all levels on one GPU, one CUDA stream each.
+    Under torchrun with WORLD_SIZE = D: one level per rank / GPU, the two level-boundary messages by NCCL send / recv.
+    A step is one solve of all levels.  Parity gate: the same code path at 32^3 against oracle/nested_oracle.py (the
+    oracle's per-level direct sums cost N^6; at the timed size they would take hours)."""
+    import torch
+    from paper_2409_02294_b200 import binding as pg, build as pg_build, nested
+    rank, local_rank, world = replicas.dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    depth, n, box0 = args.nested, (args.cart or 64), 16.0
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        if world != depth:
+            raise SystemExit(f"bench.py --nested {depth}: one level per rank needs WORLD_SIZE == {depth}, got {world}")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def level_rho(m, level, seed):
+        return make_rho3(m, 10 * seed + level)
+
+    # ---- parity gate at 32^3 (rank 0 only runs the oracle; every rank runs its level)
+    parity = {"ok": True, "what": "not run"}
+    gate_n = 32
+    gate = nested.NestedPotential(gate_n, box0, depth, device=local_rank, dist=dist)
+    g_rho = {l: torch.from_numpy(level_rho(gate_n, l, 1)).cuda() for l in gate.owned}
+    g_out = {l: torch.empty_like(g_rho[l]) for l in gate.owned}
+    gate.solve(g_rho, g_out); gate.synchronize(); gate.close()
+    if rank == 0:
+        import oracle
+        from oracle import nested_oracle
+        ref, _ = nested_oracle.nested_potential(gate_n, box0, [level_rho(gate_n, l, 1) for l in range(depth)])
+        got = g_out[0].cpu().numpy()
+        l2 = float(np.linalg.norm(got - ref[0]) / np.linalg.norm(ref[0])); mx = float(np.abs(got / ref[0] - 1).max())
+        if world == 1:
+            for l in range(1, depth):
+                g = g_out[l].cpu().numpy()
+                l2 = max(l2, float(np.linalg.norm(g - ref[l]) / np.linalg.norm(ref[l]))); mx = max(mx, float(np.abs(g / ref[l] - 1).max()))
+        parity = {"rel_l2": l2, "max_rel": mx, "bar": {"rel_l2": REL_L2, "max_rel": MAX_REL}, "ok": bool(l2 <= REL_L2 and mx <= MAX_REL),
+                  "what": f"every level this rank owns at {gate_n}^3, depth {depth}, vs oracle/nested_oracle.py (worst level)"}
+
+    # ---- timed region
+    npot = nested.NestedPotential(n, box0, depth, device=local_rank, dist=dist)
+    R = 2
+    d_rho = [{l: torch.from_numpy(level_rho(n, l, r)).cuda() for l in npot.owned} for r in range(R)]
+    d_out = [{l: torch.empty_like(d_rho[r][l]) for l in npot.owned} for r in range(R)]
+    cur = torch.cuda.current_stream()
+
+    def step(k):
+        npot.solve(d_rho[k % R], d_out[k % R])
+
+    def join():
+        for l in npot.owned:
+            cur.wait_stream(npot.levels[l].stream)
+
+    for k in range(max(3, args.warmup)):
+        step(k)
+    npot.synchronize()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    rep_ms = []
+    n0 = npot.launches()
+    for _ in range(REPEATS):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        replicas.barrier(world); torch.cuda.synchronize()
+        e0.record(cur)
+        for k in range(args.steps):
+            step(k)
+        join()
+        e1.record(cur)
+        torch.cuda.synchronize(); replicas.barrier(world)
+        rep_ms.append(replicas.max_over_ranks(e0.elapsed_time(e1), world, "cuda"))
+    n1 = npot.launches()
+    clocks = sampler.stop() if sampler is not None else None
+    ms_per_step = float(np.median(rep_ms)) / args.steps
+    h3 = pg.pg3_create(n, box0, local_rank, None)
+    alg_level = pg.pg3_algorithmic_bytes(h3)
+    pg.pg3_destroy(h3)
+    n_mean, n_halo = nested.message_counts(n)
+    alg = (2 * depth - 1) * alg_level
+    peak, peak_src = load_peaks()
+    gbs = alg / (ms_per_step * 1e-3) / 1e9 / max(1, world)
+    sane = all(bool(torch.isfinite(d_out[0][l]).all() and (d_out[0][l] < 0).all()) for l in npot.owned)
+    npot.close()
+    line = {
+        "metric": "nested-mesh solves/sec (fp64 zero-padded FFT convolution on nested 3-D meshes; row NEXT-3)",
+        "value": 1e3 / ms_per_step, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": f"{depth} nested mesh levels of {n}^3 cells (PAPER.md:267, :269, Fig. 8), box {box0:g} halved per level, "
+                               "condensed clump + 6 Gaussian clumps + 1 % noise on every level", "n": n, "depth": depth,
+                   "parallelism": (f"one level per GPU, level-boundary messages by NCCL send / recv" if world > 1
+                                   else "all levels on one GPU, one CUDA stream per level"),
+                   "exchange_bytes_per_solve": 8 * (depth - 1) * (n_mean + n_halo)},
+        "cells_per_s": depth * n**3 * 1e3 / ms_per_step, "gpu_launches": int(round((n1 - n0) / REPEATS)) * world,
+        "repeats": {"n": REPEATS, "ms_per_step_median": ms_per_step, "ms_per_step_min": min(rep_ms) / args.steps,
+                    "ms_per_step_max": max(rep_ms) / args.steps},
+        "parity": parity, "output_sane": sane,
+        "roofline": {"bound": "hbm", "kernel": f"whole path ({2 * depth - 1} single-level solves of 7 launches + coupling kernels)",
+                     "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_step": alg, "note": "per GPU"},
+        "e2e": {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                "how": "not measured for this row: densities and potentials stay resident (the paper's solver is part of a device-resident code)"},
+        "clocks": clocks,
+    }
+    if world > 1:
+        dist.barrier(); dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if not parity["ok"]:
+        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {parity}\n")
+        return 3
+    return 0
+
+
 def run_cart(args):
     """--cart N: the paper's own per-GPU workload (row NEXT-2): potential of ONE 3-D Cartesian mesh level of N^3 cells
     (N = 64 or 128) by the zero-padded FFT convolution, device resident.  Same protocol as the main
@@ -814,6 +932,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
+    ap.add_argument("--nested", type=int, default=0, help="D nested 3-D mesh levels of --cart N cells per edge (row NEXT-3; default N = 64); under torchrun with WORLD_SIZE = D one level per GPU")
     ap.add_argument("--no-fused", action="store_true", help="small grids: force the three-kernel path (PG_OPT_FUSED = 0)")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
@@ -827,6 +946,8 @@ def main():
         return run_staging(args)
     if args.pipes:
         return run_pipes(args)
+    if args.nested:
+        return run_nested(args)
     if args.cart:
         return run_cart(args)
     if args.warmup < 3 and args.impl == "ours":
