@@ -906,21 +906,26 @@ def run_cart(args):
 
 
 def run_pipes(args):
-    """--pipes: builds and runs csrc/microbench/pipes.cu (FP64 issue rate by operand pattern, FP64 || shared-memory
-    overlap, cost of scattered 16-byte accesses) -- the measurements behind the pipe model of DESIGN.md section 7."""
-    src = os.path.join(ROOT, "paper_2409_02294_b200", "csrc", "microbench", "pipes.cu")
-    exe = os.path.join(tempfile.gettempdir(), f"pg_pipes_{os.getpid()}")
-    subprocess.run([os.environ.get("NVCC", "nvcc"), "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
-    res = subprocess.run([exe], capture_output=True, text=True)
-    os.unlink(exe)
-    out = {}
-    for line in res.stdout.splitlines():
-        t = line.split()
-        if len(t) == 3 and t[0] != "status":
-            out[t[0]] = {"value": float(t[1]), "unit": t[2]}
-    print(json.dumps({"metric": "pipe microbenchmarks (csrc/microbench/pipes.cu)", "n_gpus": 1, "results": out,
-                      "status": res.stdout.strip().splitlines()[-1] if res.stdout.strip() else res.stderr[-200:]}), flush=True)
-    return res.returncode
+    """--pipes: builds and runs the microbenchmarks of csrc/microbench/ -- pipes.cu (FP64 issue rate by operand pattern,
+    FP64 || shared-memory overlap, cost of scattered 16-byte accesses) and runs.cu (what the memory system delivers for
+    transposed accesses by run length and path, STG / LDG / TMA tiles; a 16 x 16 complex transpose by shuffles against
+    shared memory) -- the measurements behind the pipe model and the design choices of DESIGN.md section 7."""
+    out, status, rc = {}, [], 0
+    for name in ("pipes.cu", "runs.cu"):
+        src = os.path.join(ROOT, "paper_2409_02294_b200", "csrc", "microbench", name)
+        exe = os.path.join(tempfile.gettempdir(), f"pg_{name[:-3]}_{os.getpid()}")
+        subprocess.run([os.environ.get("NVCC", "nvcc"), "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
+        res = subprocess.run([exe], capture_output=True, text=True)
+        os.unlink(exe)
+        for line in res.stdout.splitlines():
+            t = line.split()
+            if len(t) == 3 and t[0] != "status":
+                out[t[0]] = {"value": float(t[1]), "unit": t[2]}
+        status.append(f"{name}: " + (res.stdout.strip().splitlines()[-1] if res.stdout.strip() else res.stderr[-200:]))
+        rc = rc or res.returncode
+    print(json.dumps({"metric": "microbenchmarks (csrc/microbench/pipes.cu, runs.cu)", "n_gpus": 1, "results": out,
+                      "status": status}), flush=True)
+    return rc
 
 
 def main():
