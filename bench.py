@@ -680,7 +680,7 @@ def make_rho3(n: int, seed: int):
 
 def run_nested(args):
     """--nested D [--cart N]: the paper's distributed scheme (row NEXT-3): D nested mesh levels of N^3 cells
-    (Fig. 8 :306; readings N1-N6).  One process: all levels on one GPU, one CUDA stream each.
+    (Fig. 8 :306; readings M1-M6).  One process: all levels on one GPU, one CUDA stream each.
     Under torchrun with WORLD_SIZE = D: one level per rank / GPU, the two level-boundary messages by NCCL send / recv.
     A step is one solve of all levels.  Parity gate: the same code path at 32^3 against oracle/nested_oracle.py (the
     oracle's per-level direct sums cost N^6; at the timed size they would take hours)."""

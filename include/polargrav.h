@@ -244,20 +244,20 @@ const char *pg3_last_error(const pg3_solver *s); /* s may be NULL: last error of
 /* ---------------------------------------------------------------- nested 3-D mesh levels
  * The paper's distributed scheme: depth D nested meshes of n^3 cells with a common centre, each half the edge of the
  * one before, "each nested mesh ... allocated one GPU" (Fig. 8 :306).  PAPER.md prints no coupling
- * scheme (it is in ref. [13], :376, not available); readings N1-N6 of DESIGN.md section 3:
- *   N1  box_l = box0 / 2^l; level l+1 covers the central (n/2)^3 cells [n/4, 3n/4)^3 of level l, 2 cells per parent cell.
- *   N2  restriction, finest first: the central (n/2)^3 cells of rho_l are replaced by the means of their 8 children.
- *   N3  own_l = Phi[rho_l] and, for l < D-1, out_l = Phi[rho_l with the central cells zeroed], each the isolated
+ * scheme (it is in ref. [13], :376, not available); readings M1-M6 of DESIGN.md section 3:
+ *   M1  box_l = box0 / 2^l; level l+1 covers the central (n/2)^3 cells [n/4, 3n/4)^3 of level l, 2 cells per parent cell.
+ *   M2  restriction, finest first: the central (n/2)^3 cells of rho_l are replaced by the means of their 8 children.
+ *   M3  own_l = Phi[rho_l] and, for l < D-1, out_l = Phi[rho_l with the central cells zeroed], each the isolated
  *       single-level convolution pg3_potential computes (readings C1-C4).
- *   N4  E_0 = 0, E_(l+1) = P[out_l + E_l]: the potential of everything outside box_(l+1).
- *   N5  P: trilinear interpolation between the parent's cell centres onto the child's (weights 3/4, 1/4); the parent
+ *   M4  E_0 = 0, E_(l+1) = P[out_l + E_l]: the potential of everything outside box_(l+1).
+ *   M5  P: trilinear interpolation between the parent's cell centres onto the child's (weights 3/4, 1/4); the parent
  *       cells [n/4 - 1, 3n/4]^3 -- (n/2 + 2)^3 values -- cross the level boundary.
- *   N6  Phi_l = own_l + E_l.
+ *   M6  Phi_l = own_l + E_l.
  * One pg3n_level per level; all calls enqueue on the level's (borrowed) stream and return, except PG_MEM_HOST
  * copies, which block.  The two messages between neighbouring levels are plain device arrays the CALLER moves: by
  * pointer when both levels live on one GPU, by NCCL send / recv (NVLink) when each level has its own GPU
  * (paper_2409_02294_b200/nested.py does either).  Call order for one solve:
- *   pg3n_set_density on every level                          (copied: N2 rewrites the centre)
+ *   pg3n_set_density on every level                          (copied: M2 rewrites the centre)
  *   l = D-1 .. 1:  pg3n_restrict(l, msg) ; pg3n_absorb(l-1, msg)              msg: (n/2)^3 doubles, device
  *   every level:   pg3n_solve                                                  (independent across levels)
  *   l = 0 .. D-1:  pg3n_add_exterior(l, l ? halo : NULL) ; if l < D-1: pg3n_pack_exterior(l, halo)

@@ -1,12 +1,12 @@
 // nested.cuh -- kernels of row NEXT-3: the coupling between nested 3-D mesh levels, "each
 // nested mesh was allocated one GPU" (Fig. 8 :306).  The per-level solve is the single-level convolution
-// of cartesian.cuh; what is new here are the element-wise steps at the level boundaries (readings N1-N6 of DESIGN.md
+// of cartesian.cuh; what is new here are the element-wise steps at the level boundaries (readings M1-M6 of DESIGN.md
 // section 3; the paper prints no coupling scheme and its ref. [13] is not available):
-//   N2  restriction  fine -> coarse: mean of the 2 x 2 x 2 children, written over the parent's central (n/2)^3 cells
-//   N3  mask         the level's density with those central cells set to zero (the mass outside the child's box)
-//   N5  pack         (out_l + E_l) on the parent cells [n/4 - 1, 3n/4]^3 that cross the level boundary, (n/2 + 2)^3 values
-//   N5  prolongation trilinear interpolation of the packed parent values onto the child's cell centres, which sit at
-//                    parent coordinate n/4 + (2 i - 1)/4: weights 1/4, 3/4 (even i) or 3/4, 1/4 (odd i);  N6: Phi = own + E
+//   M2  restriction  fine -> coarse: mean of the 2 x 2 x 2 children, written over the parent's central (n/2)^3 cells
+//   M3  mask         the level's density with those central cells set to zero (the mass outside the child's box)
+//   M5  pack         (out_l + E_l) on the parent cells [n/4 - 1, 3n/4]^3 that cross the level boundary, (n/2 + 2)^3 values
+//   M5  prolongation trilinear interpolation of the packed parent values onto the child's cell centres, which sit at
+//                    parent coordinate n/4 + (2 i - 1)/4: weights 1/4, 3/4 (even i) or 3/4, 1/4 (odd i);  M6: Phi = own + E
 // All arrays [z][y][x], x fastest, fp64.  Each kernel is one pass over its output: HBM-bound, coalesced in x, and two
 // to three orders of magnitude cheaper than the solves they sit between.
 #pragma once

@@ -1662,7 +1662,7 @@ pg_status pg3n_create(pg3n_level **out, int n, double box0, int level, int depth
     pg3n_level *s = new (std::nothrow) pg3n_level;
     if (!s) { set_err3n(nullptr, "out of host memory"); return PG_ERR_NOMEM; }
     s->n = n; s->level = level; s->depth = depth;
-    pg_status rc = pg3_create(&s->mesh, n, std::ldexp(box0, -level), device, cuda_stream);   // N1: box_l = box_0 / 2^l
+    pg_status rc = pg3_create(&s->mesh, n, std::ldexp(box0, -level), device, cuda_stream);   // M1: box_l = box_0 / 2^l
     if (rc != PG_OK) { delete s; return rc; }
     s->device = s->mesh->device;
     DeviceGuard guard(s->device);
@@ -1691,7 +1691,7 @@ pg_status pg3n_set_density(pg3n_level *s, const double *rho, pg_memspace where)
     DeviceGuard guard(s->device);
     cudaStream_t st = s->mesh->inner->stream;
     const size_t bytes = (size_t)s->n * s->n * s->n * sizeof(double);
-    // always copied: N2 rewrites the central cells of every level that has a child
+    // always copied: M2 rewrites the central cells of every level that has a child
     PG3N_CUDA(s, cudaMemcpyAsync(s->d_rho, rho, bytes, where == PG_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     if (where == PG_MEM_HOST) PG3N_CUDA(s, cudaStreamSynchronize(st));
     s->have_rho = true; s->solved = false; s->have_phi = false;
@@ -1733,12 +1733,12 @@ pg_status pg3n_solve(pg3n_level *s)
     if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
     DeviceGuard guard(s->device);
     const long before = s->mesh->inner->launches;
-    pg_status rc = cart_run(s->mesh, s->d_rho, s->d_own);                                  // N3: own_l
+    pg_status rc = cart_run(s->mesh, s->d_rho, s->d_own);                                  // M3: own_l
     if (rc == PG_OK && s->level < s->depth - 1) {
         const long cells = (long)s->n * s->n * s->n;
         pgk::nest_mask_kernel<<<blocks_for(cells), 256, 0, s->mesh->inner->stream>>>(s->d_rho, s->d_mask, s->n);
         s->launches++;
-        rc = cart_run(s->mesh, s->d_mask, s->d_out);                                       // N3: out_l
+        rc = cart_run(s->mesh, s->d_mask, s->d_out);                                       // M3: out_l
     }
     if (rc != PG_OK) { snprintf(s->err, sizeof s->err, "%s", s->mesh->err); return rc; }
     PG3N_CUDA(s, cudaGetLastError());

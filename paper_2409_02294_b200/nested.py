@@ -2,7 +2,7 @@
 
 The paper runs "the convolution method ... on nested grids", one mesh level per GPU (Fig. 8 :306),
 and moves the level-boundary data with one-sided transfers.  Here every step of the arithmetic runs in
-the library's kernels (pg3n_* calls, include/polargrav.h, readings N1-N6); this module holds the SCHEDULE only:
+the library's kernels (pg3n_* calls, include/polargrav.h, readings M1-M6); this module holds the SCHEDULE only:
 
     restriction chain   l = D-1 .. 1 :  level l  --(n/2)^3 doubles-->  level l-1        (fine -> coarse)
     solves              every level, independently (own_l, out_l)
@@ -58,16 +58,16 @@ def run_schedule(levels, depth, link):
     """levels: {level index: object with restrict() -> (tensor, token), absorb(tensor, token), solve(),
     add_exterior(tensor | None, token), pack_exterior() -> (tensor, token), recv_buffers() -> (mean_like, halo_like)}
     for the levels THIS process owns; link: LocalLink or DistLink.  Every process calls this with the same depth."""
-    for l in range(depth - 1, 0, -1):                 # N2: restriction chain, finest first
+    for l in range(depth - 1, 0, -1):                 # M2: restriction chain, finest first
         if l in levels:
             t, tok = levels[l].restrict()
             link.send(l, l - 1, t, tok)
         if l - 1 in levels:
             t, tok = link.recv(l, l - 1, levels[l - 1].recv_buffers()[0])
             levels[l - 1].absorb(t, tok)
-    for l in sorted(levels):                          # N3: independent solves
+    for l in sorted(levels):                          # M3: independent solves
         levels[l].solve()
-    for l in range(depth):                            # N4-N6: exterior chain, coarsest first
+    for l in range(depth):                            # M4-M6: exterior chain, coarsest first
         if l in levels:
             if l == 0:
                 levels[l].add_exterior(None, None)

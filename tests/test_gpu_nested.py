@@ -1,4 +1,4 @@
-"""Parity of the nested-mesh path (row NEXT-3 of SURVEY.md 8(f): Fig. 8 :306; readings N1-N6)
+"""Parity of the nested-mesh path (row NEXT-3 of SURVEY.md 8(f): Fig. 8 :306; readings M1-M6)
 against oracle/nested_oracle.py, element by element on seeded densities, level by level, and of each coupling kernel
 against its oracle step.  Bar: rel-L2 <= 1e-10, max pointwise relative <= 1e-9."""
 import numpy as np
@@ -76,7 +76,7 @@ def test_coupling_kernels_step_by_step_and_call_order_errors():
             assert e.value.status == pg.PG_ERR_STATE
         pg.pg3n_restrict(h1, mean)
         pg.pg3n_synchronize(h1)
-        assert np.array_equal(mean.cpu().numpy().reshape(n // 2, n // 2, n // 2), no.restrict(fine))      # N2, same order
+        assert np.array_equal(mean.cpu().numpy().reshape(n // 2, n // 2, n // 2), no.restrict(fine))      # M2, same order
         pg.pg3n_absorb(h0, mean)
         pg.pg3n_solve(h0); pg.pg3n_solve(h1)
         pg.pg3n_add_exterior(h0, None)

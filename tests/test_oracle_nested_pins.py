@@ -1,4 +1,4 @@
-"""Pins of oracle/nested_oracle.py (NEXT-3: nested meshes, readings N1-N6 of DESIGN.md section 3).  The scheme is an
+"""Pins of oracle/nested_oracle.py (NEXT-3: nested meshes, readings M1-M6 of DESIGN.md section 3).  The scheme is an
 algorithm, so the pins fix every step against what mathematics fixes: restriction conserves mass, maps children to their parents and keeps linear fields linear,
 prolongation reproduces linear functions exactly at the children's cell centres (the +-1/4 offsets), depth 1 is the
 single-level oracle, a configuration with nothing outside the finest box has no exterior term, a far exterior point
@@ -12,7 +12,7 @@ from oracle import nested_oracle as no
 
 
 def centres(n, box, level):
-    """cell-centre coordinates of level `level` (N1): edge box / 2^level, common centre 0"""
+    """cell-centre coordinates of level `level` (M1): edge box / 2^level, common centre 0"""
     b = box / 2**level
     return -b / 2 + (np.arange(n) + 0.5) * (b / n)
 
@@ -79,7 +79,7 @@ def test_nothing_outside_the_finest_box_means_no_exterior_term():
     rng = np.random.default_rng(3)
     fine = rng.random((n, n, n))
     junk = np.zeros((n, n, n)); q = n // 4
-    junk[q:3 * q, q:3 * q, q:3 * q] = 77.0                # N2: what the caller put under the child is ignored
+    junk[q:3 * q, q:3 * q, q:3 * q] = 77.0                # M2: what the caller put under the child is ignored
     phi, rho = no.nested_potential(n, box, [junk, fine])
     assert np.array_equal(phi[1], oracle.cart_potential(n, box / 2, fine))
     assert np.array_equal(phi[0], oracle.cart_potential(n, box, no.absorb(np.zeros((n, n, n)), no.restrict(fine))))
