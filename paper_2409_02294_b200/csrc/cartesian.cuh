@@ -58,7 +58,7 @@ ycols_fwd_kernel(const cplx *__restrict__ W1, cplx *__restrict__ Yt, const cplx 
     typedef YShape<N> S;
     typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T, M = 2 * N, YM = S::YM;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     const int tid = threadIdx.x;
     const int c0 = blockIdx.x * YM;                 // columns c = kx N + z, z fastest
@@ -97,7 +97,7 @@ ycols_inv_kernel(const cplx *__restrict__ Yt, cplx *__restrict__ W1, const cplx 
     typedef YShape<N> S;
     typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T, M = 2 * N, YM = S::YM;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     const int tid = threadIdx.x;
     const int c0 = blockIdx.x * YM;
@@ -141,7 +141,7 @@ gcols_kernel(const cplx *__restrict__ src, cplx *__restrict__ dstc, double *__re
     typedef ColShape<N> S;
     typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T, M = 2 * N;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     const int tid = threadIdx.x;
     const int u = tid % T, ml = tid / T;

@@ -16,6 +16,7 @@
 //   tw_row, tw_col : compact twiddle tables (Plan<L,KIND>::TW_*), long double on the host
 #pragma once
 #include <cooperative_groups.h>
+#include <cuda.h>          // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint)
 #include "fft.cuh"
 
 #ifndef PG_ROW_THREADS
@@ -29,6 +30,9 @@
 #endif
 #ifndef PG_ROW_INLINE_FROM
 #define PG_ROW_INLINE_FROM 2048     // from this n_phi on the row kernels stage their input INSIDE the rows' own lines
+#endif
+#ifndef PG_ROW_TILE
+#define PG_ROW_TILE 1               // ... and rows_inv_kernel receives its modes as ONE 4-D TMA tile per item
 #endif
 
 namespace pgk {
@@ -64,6 +68,13 @@ struct RowShape {
     // INLINE: no staging area of its own -- the next item's input is fetched into the lines themselves once the current
     // item has left them (a shorter prefetch distance, but half the shared memory: twice the rows resident per SM)
     static constexpr bool INLINE = (NPHI >= PG_ROW_INLINE_FROM);
+    // TILE (rows_inv_kernel): the modes of an item, W[m][i0 .. i0 + ROWS) for m < L, arrive as one 4-D tensor-map copy
+    // (TMA) into the lines, laid out [m mod RA][m / RA][row]: the transposed gather in runs of ROWS x 16 bytes is done by
+    // the copy engine instead of 17 LDGSTS per thread (a quarter of the kernel's LSU wavefronts), and a quarter-warp of
+    // the row-fastest pass reads 128 contiguous bytes of the tile.  Mode L (Nyquist) comes by a plain load.
+    static constexpr bool TILE = INLINE && (PG_ROW_TILE != 0);
+    static constexpr unsigned TILE_BYTES = (unsigned)(L * ROWS * sizeof(cplx));
+    static_assert(!TILE || (L * ROWS <= ROWS * STRIDE), "the tile must fit into the lines");
     static_assert(!INLINE || SLOTS * THREADS <= ROWS * STRIDE, "the prefetch slots must fit into the lines");
     static constexpr size_t SMEM = INLINE ? (size_t)ROWS * STRIDE * sizeof(cplx) + 64
                                           : ((size_t)ROWS * STRIDE + (size_t)SLOTS * THREADS) * sizeof(cplx);
@@ -422,7 +433,7 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
                 const double *__restrict__ rscale, const int n_rows, const int n_items, const long sigma_field_stride,
                 const long w_field_stride, const int early_load)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     rows_fwd_body<NPHI, HALF, CtaBarrier>(sigma, W, tw, rscale, n_rows, n_items, sigma_field_stride, w_field_stride, early_load,
                                           blockIdx.x, gridDim.x, smem_raw);
 }
@@ -433,19 +444,37 @@ rows_fwd_kernel(const double *__restrict__ sigma, cplx *__restrict__ W, const cp
 // row, inverse pass C; the remaining passes with u fastest; multiplies row i by oscale_i
 // (= r_i^{-1/2}) and stores Phi_i.
 // HALF: only the first n_phi/2 reals of every output row are stored, in rows of that length (the crop of the x pass).
+// modes a thread of the inverse row kernel needs, by prefetch slot (the order of modes_regular / modes_special)
+template <int L>
+__device__ __forceinline__ int mode_of_slot_regular(const int slot, const int q1)
+{
+    constexpr int NB = Plan<L, ROW>::NB;
+    return (slot & 1) ? L - q1 - NB * (slot >> 1) : q1 + NB * (slot >> 1);
+}
+template <int L>
+__device__ __forceinline__ int mode_of_slot_special(const int slot)
+{
+    constexpr int NB = Plan<L, ROW>::NB;
+    if (slot < 8) return (slot & 1) ? L - NB * (slot >> 1) : NB * (slot >> 1);
+    if (slot == 8) return L / 2;
+    const int c = (slot - 9) >> 1;
+    return ((slot - 9) & 1) ? L - NB / 2 - NB * c : NB / 2 + NB * c;
+}
+
 template <int NPHI, bool HALF, class CB>
 __device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
                                               const double *__restrict__ oscale, const int n_rows, const int n_items,
                                               const long w_field_stride, const long phi_field_stride, const int block,
-                                              const int nblocks, unsigned char *smem_raw)
+                                              const int nblocks, unsigned char *smem_raw, const CUtensorMap *tmap)
 {
     typedef RowShape<NPHI> S;
     typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
-    // INLINE (RowShape): the prefetch slots lie inside the lines; the next item's modes are requested once pass A has
+    // INLINE (RowShape): the prefetched modes lie inside the lines; the next item's modes are requested once pass A has
     // taken the current item out of them and travel while pass A computes and the rows are stored
     constexpr bool INLINE = S::INLINE;
+    constexpr bool TILE = S::TILE && !HALF;
     cplx *stage = smem + (INLINE ? 0 : ROWS * S::STRIDE) + threadIdx.x;
 
     const int tid = threadIdx.x;
@@ -472,18 +501,59 @@ __device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double
     };
     auto get = [&](const int slot) { return stage[slot * S::THREADS]; };
 
+    // TILE: one tensor-map copy per item, completion on an mbarrier in the spare bytes behind the lines
+    unsigned long long *tile_bar = reinterpret_cast<unsigned long long *>(smem + ROWS * S::STRIDE);
+    cplx nyq = make_double2(0.0, 0.0);                 // mode L of row rp (special thread)
+    unsigned phase = 0;
+    auto request = [&](const int item) {               // thread 0
+        const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
+        fence_proxy_async();                           // the lines were last touched through the generic proxy
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(tile_bar)), "r"(S::TILE_BYTES) : "memory");
+        asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+                         smem_addr(smem)),
+                     "l"(tmap), "r"(2 * i0), "r"(0), "r"(0), "r"(f), "r"(smem_addr(tile_bar))
+                     : "memory");
+    };
+    auto load_nyq = [&](const int item) {
+        const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
+        return W[f * w_field_stride + (long)L * n_rows + i0 + rp];
+    };
+    auto tile_at = [&](const int k) {                  // k < L:  [k mod RA][k / RA][row]
+        return smem[((k % P::RA) * (L / P::RA) + k / P::RA) * ROWS + rp];
+    };
+    auto get_regular = [&](const int slot) { return tile_at(mode_of_slot_regular<L>(slot, q1)); };
+    auto get_special = [&](const int slot) { return slot == 1 ? nyq : tile_at(mode_of_slot_special<L>(slot)); };
+    if constexpr (TILE) {
+        if (tid == 0) mbar_init(tile_bar, 1);
+        CB::sync();
+    }
+
     pdl_wait();                    // W is written by the preceding kernel of the stream
     pdl_launch_dependents();
     int item = block;
-    if (item < n_items) prefetch(item);
+    if (item < n_items) {
+        if constexpr (TILE) {
+            if (tid == 0) request(item);
+            if (special) nyq = load_nyq(item);
+        } else {
+            prefetch(item);
+        }
+    }
     for (; item < n_items; item += nblocks) {
         const int f = item / items_per_field, i0 = (item % items_per_field) * ROWS;
         cplx v[16];
         const double sc = __ldg(&oscale[i0 + rho]);
-        cp_async_wait_all();
-        if (!special) merge_regular<L>(v, un1, get);
-        else merge_special<L>(v, un1, un2, get);
-        if constexpr (INLINE) CB::sync();     // the slots live in the lines: all of them read before pass C writes
+        if constexpr (TILE) {
+            mbar_wait(tile_bar, phase);
+            phase ^= 1;
+            if (!special) merge_regular<L>(v, un1, get_regular);
+            else merge_special<L>(v, un1, un2, get_special);
+        } else {
+            cp_async_wait_all();
+            if (!special) merge_regular<L>(v, un1, get);
+            else merge_special<L>(v, un1, un2, get);
+        }
+        if constexpr (INLINE) CB::sync();     // the modes live in the lines: all of them read before pass C writes
         else if (item + nblocks < n_items) prefetch(item + nblocks);
         inv_c_row<L>(v, smem + rp * S::STRIDE, b1, b2);
         CB::sync();
@@ -496,7 +566,14 @@ __device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double
         inv_a_load<L, ROW>(v, line, u);
         if constexpr (INLINE) {
             CB::sync();       // the lines are free: the next item's modes may land in them
-            if (item + nblocks < n_items) prefetch(item + nblocks);
+            if (item + nblocks < n_items) {
+                if constexpr (TILE) {
+                    if (tid == 0) request(item + nblocks);
+                    if (special) nyq = load_nyq(item + nblocks);
+                } else {
+                    prefetch(item + nblocks);
+                }
+            }
         }
         inv_a_compute<L, ROW>(v, bases, u);
         cplx *y = reinterpret_cast<cplx *>(phi + f * phi_field_stride + (long)(i0 + rho) * (HALF ? NPHI / 2 : NPHI));
@@ -509,11 +586,11 @@ template <int NPHI, bool HALF = false>
 __global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
 rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
                 const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
-                const long phi_field_stride)
+                const long phi_field_stride, const __grid_constant__ CUtensorMap tmap)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     rows_inv_body<NPHI, HALF, CtaBarrier>(W, phi, tw, oscale, n_rows, n_items, w_field_stride, phi_field_stride, blockIdx.x,
-                                          gridDim.x, smem_raw);
+                                          gridDim.x, smem_raw, &tmap);
 }
 
 // thread of a column transform that holds the mirror bins of thread u: bin0(partner) = T - bin0(u)  (u != 0)
@@ -622,7 +699,7 @@ __global__ void __launch_bounds__(ColShape<NR>::THREADS, ColShape<NR>::MIN_CTAS)
 cols_kernel(cplx *__restrict__ W, const double *__restrict__ Khat, const cplx *__restrict__ tw, const int n_modes,
             const long w_field_stride)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cols_body<NR, CtaBarrier>(W, Khat, tw, n_modes, w_field_stride, blockIdx.x, blockIdx.y, smem_raw);
 }
 
@@ -651,7 +728,7 @@ fused_solve_kernel(const double *__restrict__ sigma, double *__restrict__ phi, c
     typedef FusedShape<NR, NPHI> F;
     typedef typename F::RS RS;
     typedef typename F::CS CS;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const int n_items = (NR / RS::ROWS) * batch;
     constexpr int n_modes = NPHI / 2 + 1;
@@ -668,7 +745,7 @@ fused_solve_kernel(const double *__restrict__ sigma, double *__restrict__ phi, c
     grid.sync();
     if (threadIdx.x < RS::THREADS)
         rows_inv_body<NPHI, false, PartBarrier<RS::THREADS>>(W, phi, tw_row, oscale, NR, n_items, w_field_stride,
-                                                            field_stride, blockIdx.x, gridDim.x, smem_raw);
+                                                            field_stride, blockIdx.x, gridDim.x, smem_raw, nullptr);
 }
 
 // ---------------------------------------------------------------- a1: Green's kernel
@@ -703,7 +780,7 @@ khat_cols_kernel(const cplx *__restrict__ WK, double *__restrict__ Khat, const c
     constexpr int L = 2 * NR;
     typedef Plan<L, COL> P;
     constexpr int T = P::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *line = reinterpret_cast<cplx *>(smem_raw);
 
     const int u = threadIdx.x;
@@ -740,7 +817,7 @@ direct_kernel(const double *__restrict__ sigma, double *__restrict__ phi, const 
               const double *__restrict__ dA, const double *__restrict__ s2, const int n_r, const int n_phi,
               const double eps2, const int ring0, const long sigma_field_stride, const long phi_field_stride)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     double *w = reinterpret_cast<double *>(smem_raw);   // [n_phi] Sigma of the source ring
     double *g = w + n_phi;                              // [n_phi] pair kernel by azimuthal lag
     const int i = ring0 + blockIdx.x;
@@ -802,7 +879,7 @@ direct_tiled_kernel(const double *__restrict__ sigma, double *__restrict__ phi, 
 {
     static_assert(R % 8 == 0 && R >= 8 && R <= 16, "targets per thread");
     constexpr int NG = R / 8 + 1;                       // groups of 8 lags in the window
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     double *w = reinterpret_cast<double *>(smem_raw);   // [n_phi] Sigma of the source ring
     double *g = w + n_phi;                              // [2 n_phi / R][R + 2] pair kernel by lag, twice over
     auto slot = [](const int lag) { return (lag / R) * (R + 2) + lag % R; };

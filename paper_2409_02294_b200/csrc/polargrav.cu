@@ -11,6 +11,7 @@
 #include "nested.cuh"
 
 #include <cmath>
+#include <cudaTypedefs.h>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
@@ -26,6 +27,10 @@ namespace {
 
 constexpr int kMaxProfiledCalls = 2048;
 
+#ifndef PG_TMAP_L2
+#define PG_TMAP_L2 CU_TENSOR_MAP_L2_PROMOTION_NONE   // L2 promotion of the tile loads (128B / 256B tried: no difference)
+#endif
+
 thread_local char g_create_error[512] = "";
 
 struct Events4 { cudaEvent_t e[4]; };
@@ -37,6 +42,9 @@ struct pg_solver {
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
     int sm_count = 0, row_ctas = 0;   // persistent grid of the row kernels
     // small grids (64 .. 512 per axis): the whole solve in one cooperative launch (kernels.cuh, fused_solve_kernel)
+    // tensor maps of the W buffers rows_inv_kernel reads as 4-D TMA tiles (n_phi >= PG_ROW_INLINE_FROM), by buffer
+    struct RowTmap { const void *base; int n_rows, fields; long stride; CUtensorMap map; };
+    std::vector<RowTmap> row_tmaps;
     int fused = 1;                    // PG_OPT_FUSED
     int fused_cap = 0;                // CTAs of the fused kernel resident at once (0: the grid has no fused kernel)
     int fused_items = 0, fused_groups = 0;   // row items and mode groups per field
@@ -271,6 +279,52 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
     return PG_OK;
 }
 
+// Tensor map of a W buffer for the tile loads of rows_inv_kernel (kernels.cuh, RowShape::TILE): as doubles,
+//   dim 0  2 n_rows (one column of W, contiguous)           box 2 ROWS   (one run of ROWS rows)
+//   dim 1  a = m / RA, L / RA values, stride RA columns      box L / RA
+//   dim 2  c = m mod RA, RA values, stride one column        box RA       -> tile [c][a][row] in shared memory
+//   dim 3  field                                             box 1
+// Mode L (the 1025th column at n_phi = 2048) is outside the map and fetched by a plain load.
+template <int NPHI>
+pg_status row_tmap(pg_solver *s, const cplx *Z, int n_rows, int fields, long z_stride, CUtensorMap *out)
+{
+    typedef pgk::RowShape<NPHI> S;
+    typedef pgk::Plan<S::L, pgk::ROW> P;
+    memset(out, 0, sizeof *out);
+    if constexpr (!S::TILE) {
+        (void)s; (void)Z; (void)n_rows; (void)fields; (void)z_stride;
+        return PG_OK;
+    } else {
+        for (const auto &e : s->row_tmaps)
+            if (e.base == Z && e.n_rows == n_rows && e.fields == fields && e.stride == z_stride) { *out = e.map; return PG_OK; }
+        static PFN_cuTensorMapEncodeTiled encode = nullptr;
+        if (!encode) {
+            void *fn = nullptr;
+            cudaDriverEntryPointQueryResult q;
+            if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+                q != cudaDriverEntryPointSuccess || !fn) {
+                set_err(s, "cuTensorMapEncodeTiled is not available from this driver");
+                return PG_ERR_CUDA;
+            }
+            encode = (PFN_cuTensorMapEncodeTiled)fn;
+        }
+        const cuuint64_t dims[4] = {2ull * (cuuint64_t)n_rows, (cuuint64_t)(S::L / P::RA), (cuuint64_t)P::RA, (cuuint64_t)fields};
+        const cuuint64_t strides[3] = {(cuuint64_t)P::RA * n_rows * sizeof(cplx), (cuuint64_t)n_rows * sizeof(cplx),
+                                       (cuuint64_t)z_stride * sizeof(cplx)};
+        const cuuint32_t box[4] = {2u * S::ROWS, (cuuint32_t)(S::L / P::RA), (cuuint32_t)P::RA, 1u};
+        const cuuint32_t es[4] = {1, 1, 1, 1};
+        pg_solver::RowTmap e{Z, n_rows, fields, z_stride, {}};
+        const CUresult r = encode(&e.map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<cplx *>(Z), dims, strides, box, es,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, PG_TMAP_L2,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { set_err(s, "cuTensorMapEncodeTiled failed (%d)", (int)r); return PG_ERR_CUDA; }
+        if (s->row_tmaps.size() >= 64) s->row_tmaps.clear();
+        s->row_tmaps.push_back(e);
+        *out = e.map;
+        return PG_OK;
+    }
+}
+
 template <int NPHI>
 pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, long z_stride, long phi_stride,
                           cudaStream_t st, const double *oscale)
@@ -278,8 +332,11 @@ pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, l
     typedef pgk::RowShape<NPHI> S;
     const int n_items = (s->n_r / S::ROWS) * batch;
     const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
+    CUtensorMap tmap;
+    pg_status rc = row_tmap<NPHI>(s, Z, s->n_r, batch, z_stride, &tmap);
+    if (rc != PG_OK) return rc;
     PG_CUDA(s, launch_pdl(pgk::rows_inv_kernel<NPHI>, dim3(grid), dim3(S::THREADS), S::SMEM, st, Z, phi, s->d_tw_row,
-                          oscale, s->n_r, n_items, z_stride, phi_stride));
+                          oscale, s->n_r, n_items, z_stride, phi_stride, tmap));
     note_early_release_output(s->device, st, phi, (size_t)s->n_r * NPHI * sizeof(double) * batch);
     s->launches++;
     return PG_OK;
@@ -1437,7 +1494,7 @@ pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
     in->launches++;
     // inverse x pass, cropped to the first N reals of every row: Phi[z][y][x]
     PG3_CUDA(s, launch_pdl(pgk::rows_inv_kernel<M, true>, dim3(rgrid), dim3(RS::THREADS), RS::SMEM, st, (const cplx *)in->d_W,
-                           d_phi, (const cplx *)in->d_tw_row, (const double *)s->d_ones, N, n_items, ws, (long)N * N));
+                           d_phi, (const cplx *)in->d_tw_row, (const double *)s->d_ones, N, n_items, ws, (long)N * N, CUtensorMap{}));
     in->launches++;
     PG3_CUDA(s, cudaGetLastError());
     return PG_OK;

@@ -50,7 +50,7 @@ khat_cols_cplx_kernel(const cplx *__restrict__ WK, cplx *__restrict__ KhatC, con
     constexpr int L = 2 * NR;
     typedef Plan<L, COL> P;
     constexpr int T = P::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *line = reinterpret_cast<cplx *>(smem_raw);
     const int u = threadIdx.x;
     const int m = blockIdx.x;
@@ -81,7 +81,7 @@ cols_cplx_kernel(const cplx *__restrict__ Wsrc, cplx *__restrict__ Wdst, const c
     typedef ColShape<NR> S;
     typedef Plan<S::L, COL> P;
     constexpr int L = S::L, T = S::T;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
     const int tid = threadIdx.x;
     const int u = tid % T, ml = tid / T;
