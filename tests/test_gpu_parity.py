@@ -426,3 +426,31 @@ def test_resident_and_staged_solves_interleaved_with_the_option_on():
         pin_in.free(); pin_out.free()
     finally:
         d.close()
+
+
+@pytest.mark.parametrize("n_r,batch", [(64, 1), (256, 3)])
+def test_wide_rows_with_few_rings_and_a_batch(n_r, batch):
+    """n_phi = 2048 takes the 4-row row kernels with in-line staging and, in the inverse row kernel, one TMA tile per item
+    (tensor map over [field][mode][ring]): few rings (a handful of items per field) and a batch (the field dimension of
+    the map) against the oracle on every cell, and the batch against single solves bit for bit."""
+    n_phi, r_in, r_out, eps = 2048, 1.0, 40.0, 0.01
+    sig = np.stack([random_sigma(n_r, n_phi, 8100 + b) for b in range(batch)])
+    s = pg.Solver(n_r, n_phi, r_in, r_out, eps, max_batch=batch, device=0,
+                  cuda_stream=torch.cuda.current_stream().cuda_stream)
+    try:
+        d_s = torch.from_numpy(sig).cuda()
+        d_p = torch.empty_like(d_s)
+        pg.pg_set_density(s.h, d_s, batch, pg.PG_MEM_DEVICE)
+        pg.pg_potential(s.h, d_p, batch, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(s.h)
+        got = d_p.cpu().numpy()
+        for b in range(batch):
+            ref = oracle.potential_o1(n_r, n_phi, r_in, r_out, eps, sig[b])
+            assert_parity(got[b], ref, f"{n_r}x{n_phi} field {b}")
+            one = torch.empty_like(d_s[b:b + 1])
+            pg.pg_set_density(s.h, d_s[b:b + 1].contiguous(), 1, pg.PG_MEM_DEVICE)
+            pg.pg_potential(s.h, one, 1, pg.PG_MEM_DEVICE)
+            pg.pg_synchronize(s.h)
+            assert np.array_equal(one.cpu().numpy()[0], got[b])
+    finally:
+        s.close()
