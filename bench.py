@@ -440,6 +440,9 @@ def run_ours(args):
             "traffic_source": (f"profiles/ncu_head.json, ncu --set full at commit {ncu['commit']}" if ncu else ncu_why),
             "peak_source": peak_src,
             "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
+            "algorithmic_bytes_note": "SURVEY.md 8(d)'s figures (56 B/cell; the 49.0 us target derives from them). The column "
+                                      "kernel reads Khat as its symmetric half, so it needs 8 N_r M_h bytes less than counted here "
+                                      "(84.0 instead of 100.8 MB at 2048^2); DRAM traffic per launch is in `traffic`.",
             "kernels": {pg.KERNEL_NAMES[i]: {"ms": per_launch_ms[i], "alg_bytes": kbytes[i],
                                             "gbs": kbytes[i] / (per_launch_ms[i] * 1e-3) / 1e9 if per_launch_ms[i] > 0 else None}
                         for i in range(pg.PG_NUM_KERNELS)},
