@@ -709,7 +709,8 @@ def run_nested(args):
     # ---- parity gate at 32^3 (rank 0 only runs the oracle; every rank runs its level)
     parity = {"ok": True, "what": "not run"}
     gate_n = 32
-    gate = nested.NestedPotential(gate_n, box0, depth, device=local_rank, dist=dist)
+    link_kw = dict(link=args.nested_link, token_device=(f"cuda:{local_rank}" if world > 1 else "cpu"))
+    gate = nested.NestedPotential(gate_n, box0, depth, device=local_rank, dist=dist, **link_kw)
     g_rho = {l: torch.from_numpy(level_rho(gate_n, l, 1)).cuda() for l in gate.owned}
     g_out = {l: torch.empty_like(g_rho[l]) for l in gate.owned}
     gate.solve(g_rho, g_out); gate.synchronize(); gate.close()
@@ -727,7 +728,7 @@ def run_nested(args):
                   "what": f"every level this rank owns at {gate_n}^3, depth {depth}, vs oracle/nested_oracle.py (worst level)"}
 
     # ---- timed region
-    npot = nested.NestedPotential(n, box0, depth, device=local_rank, dist=dist)
+    npot = nested.NestedPotential(n, box0, depth, device=local_rank, dist=dist, **link_kw)
     R = 2
     d_rho = [{l: torch.from_numpy(level_rho(n, l, r)).cuda() for l in npot.owned} for r in range(R)]
     d_out = [{l: torch.empty_like(d_rho[r][l]) for l in npot.owned} for r in range(R)]
@@ -775,7 +776,9 @@ def run_nested(args):
         "data": "synthetic",
         "config": {"workload": f"{depth} nested mesh levels of {n}^3 cells (PAPER.md:267, :269, Fig. 8), box {box0:g} halved per level, "
                                "condensed clump + 6 Gaussian clumps + 1 % noise on every level", "n": n, "depth": depth,
-                   "parallelism": (f"one level per GPU, level-boundary messages by NCCL send / recv" if world > 1
+                   "parallelism": ((f"one level per GPU, level-boundary messages "
+                                    + ("PUT by the producing kernels into the neighbour's inbox (CUDA IPC peer memory), nccl tokens"
+                                       if args.nested_link == "put" else "by NCCL send / recv")) if world > 1
                                    else "all levels on one GPU, one CUDA stream per level"),
                    "exchange_bytes_per_solve": 8 * (depth - 1) * (n_mean + n_halo)},
         "cells_per_s": depth * n**3 * 1e3 / ms_per_step, "gpu_launches": int(round((n1 - n0) / REPEATS)) * world,
@@ -941,6 +944,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
     ap.add_argument("--nested", type=int, default=0, help="D nested 3-D mesh levels of --cart N cells per edge (row NEXT-3; default N = 64); under torchrun with WORLD_SIZE = D one level per GPU")
+    ap.add_argument("--nested-link", default="put", choices=["put", "sendrecv"],
+                    help="--nested under torchrun: one-sided puts into the neighbours' inboxes (default) or NCCL send / recv of the messages")
     ap.add_argument("--no-fused", action="store_true", help="small grids: force the three-kernel path (PG_OPT_FUSED = 0)")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],

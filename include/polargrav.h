@@ -264,7 +264,26 @@ const char *pg3_last_error(const pg3_solver *s); /* s may be NULL: last error of
  *                                                                              halo: (n/2 + 2)^3 doubles, device
  *   pg3n_potential on every level.
  * n in {32, 64, 128, 256}; device pointers 16-byte aligned.  PG_ERR_STATE for calls out of order or on the wrong end
- * of the hierarchy (restrict on level 0, absorb / pack on the finest level). */
+ * of the hierarchy (restrict on level 0, absorb / pack on the finest level).
+ *
+ * One-sided exchange.  The paper's images move level-boundary data by one-sided transfers: "one image is allowed to
+ * access the data from another without any action from the target image" (section 2.5).  The same here:
+ * every level owns two INBOXES (device arrays of the two message sizes); a neighbour opens them -- by CUDA IPC handle
+ * from another process / GPU (peer access over NVLink is enabled on open), or by plain pointer inside one process --
+ * and the kernels of pg3n_restrict / pg3n_pack_exterior then write their message STRAIGHT INTO the neighbour's inbox:
+ * the transfer is the kernel's own stores, no copy kernel, no staging.  Pass NULL where the calls above take a message
+ * pointer:  pg3n_restrict(l, NULL) puts into the parent's MEAN inbox, pg3n_absorb(l, NULL) reads this level's MEAN
+ * inbox, pg3n_pack_exterior(l, NULL) puts into the child's HALO inbox, pg3n_add_exterior(l > 0, NULL) reads this
+ * level's HALO inbox.  The library does not signal: the sender's stream must have completed the putting kernel before
+ * the receiver is told to go on (nested.py: event synchronise, then a one-byte message), and the receiver must have
+ * consumed an inbox before the next put into it (guaranteed by the order of the two chains within a solve).
+ *   pg3n_inbox_export  allocates the inbox on first use; returns its IPC handle (64 bytes; may be NULL) and its
+ *                      device address (may be NULL).  PG_ERR_STATE if the level receives no such message.
+ *   pg3n_peer_open     opens the NEIGHBOUR's inbox from its handle: MEAN = the parent's (target of pg3n_restrict),
+ *                      HALO = the child's (target of pg3n_pack_exterior).  pg3n_peer_set: same, by device pointer.
+ */
+#define PG_IPC_HANDLE_BYTES 64
+typedef enum { PG3N_INBOX_MEAN = 0, PG3N_INBOX_HALO = 1 } pg3n_inbox;
 typedef struct pg3n_level pg3n_level; /* opaque */
 pg_status pg3n_create(pg3n_level **out, int n, double box0, int level, int depth, int device, void *cuda_stream);
 pg_status pg3n_set_density(pg3n_level *s, const double *rho, pg_memspace where);
@@ -274,6 +293,9 @@ pg_status pg3n_solve(pg3n_level *s);
 pg_status pg3n_add_exterior(pg3n_level *s, const double *parent_halo);
 pg_status pg3n_pack_exterior(pg3n_level *s, double *halo_out);
 pg_status pg3n_potential(pg3n_level *s, double *phi, pg_memspace where);
+pg_status pg3n_inbox_export(pg3n_level *s, pg3n_inbox which, unsigned char handle[PG_IPC_HANDLE_BYTES], double **local_ptr);
+pg_status pg3n_peer_open(pg3n_level *s, pg3n_inbox which, const unsigned char handle[PG_IPC_HANDLE_BYTES]);
+pg_status pg3n_peer_set(pg3n_level *s, pg3n_inbox which, double *neighbour_inbox);
 pg_status pg3n_synchronize(pg3n_level *s);
 pg_status pg3n_destroy(pg3n_level *s); /* pg3n_destroy(NULL) is a no-op returning PG_OK */
 long pg3n_launch_count(const pg3n_level *s);

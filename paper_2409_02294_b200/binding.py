@@ -35,6 +35,7 @@ EXPORTS = (
     "pg3_algorithmic_bytes", "pg3_last_error",
     "pg3n_create", "pg3n_set_density", "pg3n_restrict", "pg3n_absorb", "pg3n_solve", "pg3n_add_exterior",
     "pg3n_pack_exterior", "pg3n_potential", "pg3n_synchronize", "pg3n_destroy", "pg3n_launch_count", "pg3n_last_error",
+    "pg3n_inbox_export", "pg3n_peer_open", "pg3n_peer_set",
 )
 
 _lib = None
@@ -89,6 +90,9 @@ def lib():
         L.pg3n_potential.argtypes = [vp, vp, i]
         L.pg3n_synchronize.argtypes = [vp]
         L.pg3n_destroy.argtypes = [vp]
+        L.pg3n_inbox_export.argtypes = [vp, i, ctypes.c_char_p, ctypes.POINTER(vp)]
+        L.pg3n_peer_open.argtypes = [vp, i, ctypes.c_char_p]
+        L.pg3n_peer_set.argtypes = [vp, i, vp]
         for name in EXPORTS:
             getattr(L, name).restype = i
         L.pg3n_launch_count.argtypes = [vp]; L.pg3n_launch_count.restype = l
@@ -324,6 +328,28 @@ def pg3n_synchronize(h):
 
 def pg3n_destroy(h):
     _check3n(lib().pg3n_destroy(h))
+
+
+PG3N_INBOX_MEAN, PG3N_INBOX_HALO = 0, 1
+PG_IPC_HANDLE_BYTES = 64
+
+
+def pg3n_inbox_export(h, which):
+    """(IPC handle as 64 bytes, device address) of this level's inbox `which`; allocates it on first use."""
+    buf = ctypes.create_string_buffer(PG_IPC_HANDLE_BYTES)
+    ptr = ctypes.c_void_p()
+    _check3n(lib().pg3n_inbox_export(h, which, buf, ctypes.byref(ptr)), h)
+    return buf.raw, ptr.value
+
+
+def pg3n_peer_open(h, which, handle: bytes):
+    if len(handle) != PG_IPC_HANDLE_BYTES:
+        raise ValueError("an IPC handle has 64 bytes")
+    _check3n(lib().pg3n_peer_open(h, which, handle), h)
+
+
+def pg3n_peer_set(h, which, device_address):
+    _check3n(lib().pg3n_peer_set(h, which, device_address), h)
 
 
 def pg3n_launch_count(h):

@@ -1663,6 +1663,11 @@ struct pg3n_level {
     pg3_solver *mesh = nullptr;
     double *d_rho = nullptr, *d_mask = nullptr, *d_own = nullptr, *d_out = nullptr, *d_ext = nullptr, *d_phi = nullptr;
     bool have_rho = false, solved = false, have_phi = false;
+    // one-sided exchange: this level's two inboxes (owned, cudaMalloc'ed so that they can be exported to
+    // another process) and the neighbours' inboxes it puts into ([0] the parent's MEAN inbox, [1] the child's HALO inbox)
+    double *inbox[2] = {nullptr, nullptr};
+    double *peer[2] = {nullptr, nullptr};
+    bool peer_ipc[2] = {false, false};
     long launches = 0;
     char err[512] = "";
 };
@@ -1699,6 +1704,10 @@ void nest_free(pg3n_level *s)
 {
     if (!s) return;
     cudaFree(s->d_rho); cudaFree(s->d_mask); cudaFree(s->d_own); cudaFree(s->d_out); cudaFree(s->d_ext); cudaFree(s->d_phi);
+    for (int k = 0; k < 2; ++k) {
+        if (s->peer[k] && s->peer_ipc[k]) cudaIpcCloseMemHandle(s->peer[k]);
+        cudaFree(s->inbox[k]);
+    }
     if (s->mesh) pg3_destroy(s->mesh);
     delete s;
 }
@@ -1760,6 +1769,10 @@ pg_status pg3n_restrict(pg3n_level *s, double *child_mean_out)
     if (!s) return PG_ERR_INVALID_ARG;
     if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
     if (s->level == 0) { set_err3n(s, "level 0 has no parent to restrict to"); return PG_ERR_STATE; }
+    if (!child_mean_out) {                     // one-sided: straight into the parent's inbox (peer memory)
+        if (!s->peer[PG3N_INBOX_MEAN]) { set_err3n(s, "pg3n_restrict(NULL): the parent's inbox has not been opened (pg3n_peer_open / pg3n_peer_set)"); return PG_ERR_STATE; }
+        child_mean_out = s->peer[PG3N_INBOX_MEAN];
+    }
     if (!dev_ptr_ok(s, child_mean_out, "child_mean_out")) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
     const long q = s->n / 2;
@@ -1774,6 +1787,10 @@ pg_status pg3n_absorb(pg3n_level *s, const double *child_mean)
     if (!s) return PG_ERR_INVALID_ARG;
     if (!s->have_rho) { set_err3n(s, "no density set"); return PG_ERR_STATE; }
     if (s->level == s->depth - 1) { set_err3n(s, "the finest level has no child to absorb"); return PG_ERR_STATE; }
+    if (!child_mean) {                         // one-sided: what the child has put into this level's inbox
+        if (!s->inbox[PG3N_INBOX_MEAN]) { set_err3n(s, "pg3n_absorb(NULL): this level has no MEAN inbox (pg3n_inbox_export)"); return PG_ERR_STATE; }
+        child_mean = s->inbox[PG3N_INBOX_MEAN];
+    }
     if (!dev_ptr_ok(s, child_mean, "child_mean")) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
     const long q = s->n / 2;
@@ -1809,6 +1826,10 @@ pg_status pg3n_add_exterior(pg3n_level *s, const double *parent_halo)
     if (!s) return PG_ERR_INVALID_ARG;
     if (!s->solved) { set_err3n(s, "pg3n_add_exterior before pg3n_solve"); return PG_ERR_STATE; }
     if (s->level == 0 && parent_halo) { set_err3n(s, "level 0 is isolated: parent_halo must be NULL"); return PG_ERR_INVALID_ARG; }
+    if (s->level > 0 && !parent_halo) {        // one-sided: what the parent has put into this level's inbox
+        if (!s->inbox[PG3N_INBOX_HALO]) { set_err3n(s, "parent_halo is NULL and this level has no HALO inbox (pg3n_inbox_export)"); return PG_ERR_INVALID_ARG; }
+        parent_halo = s->inbox[PG3N_INBOX_HALO];
+    }
     if (s->level > 0 && !dev_ptr_ok(s, parent_halo, "parent_halo")) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
     const long cells = (long)s->n * s->n * s->n;
@@ -1824,6 +1845,10 @@ pg_status pg3n_pack_exterior(pg3n_level *s, double *halo_out)
     if (!s) return PG_ERR_INVALID_ARG;
     if (!s->have_phi) { set_err3n(s, "pg3n_pack_exterior before pg3n_add_exterior"); return PG_ERR_STATE; }
     if (s->level == s->depth - 1) { set_err3n(s, "the finest level has no child"); return PG_ERR_STATE; }
+    if (!halo_out) {                           // one-sided: straight into the child's inbox (peer memory)
+        if (!s->peer[PG3N_INBOX_HALO]) { set_err3n(s, "pg3n_pack_exterior(NULL): the child's inbox has not been opened (pg3n_peer_open / pg3n_peer_set)"); return PG_ERR_STATE; }
+        halo_out = s->peer[PG3N_INBOX_HALO];
+    }
     if (!dev_ptr_ok(s, halo_out, "halo_out")) return PG_ERR_INVALID_ARG;
     DeviceGuard guard(s->device);
     const long m = s->n / 2 + 2;
@@ -1848,6 +1873,62 @@ pg_status pg3n_potential(pg3n_level *s, double *phi, pg_memspace where)
     PG3N_CUDA(s, cudaMemcpyAsync(phi, s->d_phi, bytes, where == PG_MEM_DEVICE ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
     if (where == PG_MEM_HOST) PG3N_CUDA(s, cudaStreamSynchronize(st));
     return PG_OK;
+}
+
+pg_status pg3n_inbox_export(pg3n_level *s, pg3n_inbox which, unsigned char handle[PG_IPC_HANDLE_BYTES], double **local_ptr)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (which != PG3N_INBOX_MEAN && which != PG3N_INBOX_HALO) { set_err3n(s, "unknown inbox %d", (int)which); return PG_ERR_INVALID_ARG; }
+    if ((which == PG3N_INBOX_MEAN && s->level == s->depth - 1) || (which == PG3N_INBOX_HALO && s->level == 0)) {
+        set_err3n(s, "level %d of %d receives no such message", s->level, s->depth);
+        return PG_ERR_STATE;
+    }
+    static_assert(sizeof(cudaIpcMemHandle_t) == PG_IPC_HANDLE_BYTES, "IPC handle size");
+    DeviceGuard guard(s->device);
+    if (!s->inbox[which]) {
+        const long m = which == PG3N_INBOX_MEAN ? s->n / 2 : s->n / 2 + 2;
+        PG3N_CUDA(s, cudaMalloc((void **)&s->inbox[which], (size_t)(m * m * m) * sizeof(double)));
+    }
+    if (handle) {
+        cudaIpcMemHandle_t hnd;
+        PG3N_CUDA(s, cudaIpcGetMemHandle(&hnd, s->inbox[which]));
+        memcpy(handle, &hnd, sizeof hnd);
+    }
+    if (local_ptr) *local_ptr = s->inbox[which];
+    return PG_OK;
+}
+
+static pg_status peer_replace(pg3n_level *s, pg3n_inbox which, double *ptr, bool ipc)
+{
+    if (s->peer[which] && s->peer_ipc[which]) PG3N_CUDA(s, cudaIpcCloseMemHandle(s->peer[which]));
+    s->peer[which] = ptr;
+    s->peer_ipc[which] = ipc;
+    return PG_OK;
+}
+
+pg_status pg3n_peer_open(pg3n_level *s, pg3n_inbox which, const unsigned char handle[PG_IPC_HANDLE_BYTES])
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!handle || (which != PG3N_INBOX_MEAN && which != PG3N_INBOX_HALO)) { set_err3n(s, "pg3n_peer_open: bad argument"); return PG_ERR_INVALID_ARG; }
+    if ((which == PG3N_INBOX_MEAN && s->level == 0) || (which == PG3N_INBOX_HALO && s->level == s->depth - 1)) {
+        set_err3n(s, "level %d of %d sends no such message", s->level, s->depth);
+        return PG_ERR_STATE;
+    }
+    DeviceGuard guard(s->device);
+    cudaIpcMemHandle_t hnd;
+    memcpy(&hnd, handle, sizeof hnd);
+    void *p = nullptr;
+    PG3N_CUDA(s, cudaIpcOpenMemHandle(&p, hnd, cudaIpcMemLazyEnablePeerAccess));
+    return peer_replace(s, which, (double *)p, true);
+}
+
+pg_status pg3n_peer_set(pg3n_level *s, pg3n_inbox which, double *neighbour_inbox)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (which != PG3N_INBOX_MEAN && which != PG3N_INBOX_HALO) { set_err3n(s, "unknown inbox %d", (int)which); return PG_ERR_INVALID_ARG; }
+    if (neighbour_inbox && !dev_ptr_ok(s, neighbour_inbox, "neighbour_inbox")) return PG_ERR_INVALID_ARG;
+    DeviceGuard guard(s->device);
+    return peer_replace(s, which, neighbour_inbox, false);
 }
 
 pg_status pg3n_synchronize(pg3n_level *s)

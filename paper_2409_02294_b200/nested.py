@@ -12,7 +12,10 @@ the library's kernels (pg3n_* calls, include/polargrav.h, readings M1-M6); this 
   * all levels of one process on ONE GPU, one CUDA stream per level (the "CUDA Streams" the paper leaves unexplored,
     PAPER.md:269): messages are handed over by pointer, ordered by stream events (`LocalLink`);
   * one level per rank / GPU: messages travel by `torch.distributed` send / recv -- NCCL over NVLink on GPUs
-    (`DistLink`); the solves of the levels then run concurrently on their own GPUs.
+    (`DistLink`) -- or ONE-SIDED (`PutLink`, the paper's own model): every level exports its two inboxes by
+    CUDA IPC handle, its neighbours open them, and the restriction / packing kernels write their message straight into
+    the neighbour's inbox (peer stores over NVLink); all that travels through `torch.distributed` is a one-element
+    "it is there" token.  The solves of the levels run concurrently on their own GPUs.
 The world-size-2 gloo test drives the same schedule on CPU tensors with stand-in levels (tests/test_multirank_gloo.py).
 No arithmetic of the method lives here.
 """
@@ -54,6 +57,41 @@ class DistLink:
         return like, None
 
 
+class PutLink:
+    """One level per rank, one-sided: the payload has been PUT into the receiver's inbox by the sender's kernel; send /
+    recv move a one-element token that tells the receiver so.  `connect` exchanges the IPC handles once."""
+
+    def __init__(self, dist, group=None, token_device="cpu"):
+        import torch
+        self.dist, self.group = dist, group
+        self.tok = torch.zeros(1, dtype=torch.int32, device=token_device)
+
+    def connect(self, level):
+        """level: the GpuLevel this rank owns (rank = level index)."""
+        pg = level.pg
+        mine = {}
+        if level.level < level.depth - 1:
+            mine["mean"] = pg.pg3n_inbox_export(level.h, pg.PG3N_INBOX_MEAN)[0]
+        if level.level > 0:
+            mine["halo"] = pg.pg3n_inbox_export(level.h, pg.PG3N_INBOX_HALO)[0]
+        everyone = [None] * self.dist.get_world_size(self.group)
+        self.dist.all_gather_object(everyone, mine, group=self.group)
+        if level.level > 0:                                   # restriction goes into the parent's MEAN inbox
+            pg.pg3n_peer_open(level.h, pg.PG3N_INBOX_MEAN, everyone[level.level - 1]["mean"])
+        if level.level < level.depth - 1:                     # the exterior potential into the child's HALO inbox
+            pg.pg3n_peer_open(level.h, pg.PG3N_INBOX_HALO, everyone[level.level + 1]["halo"])
+        level.one_sided = True
+
+    def send(self, src_level, dst_level, tensor, token=None):
+        if token is not None:
+            token.synchronize()                       # the putting kernel has completed: the message is in the inbox
+        self.dist.send(self.tok, dst=dst_level, group=self.group)
+
+    def recv(self, src_level, dst_level, like=None):
+        self.dist.recv(self.tok, src=src_level, group=self.group)
+        return None, None
+
+
 def run_schedule(levels, depth, link):
     """levels: {level index: object with restrict() -> (tensor, token), absorb(tensor, token), solve(),
     add_exterior(tensor | None, token), pack_exterior() -> (tensor, token), recv_buffers() -> (mean_like, halo_like)}
@@ -93,6 +131,7 @@ class GpuLevel:
             n_mean, n_halo = message_counts(n)
             mk = lambda c: torch.empty(c, dtype=torch.float64, device=f"cuda:{device}")
             self.mean_out, self.halo_out, self.mean_in, self.halo_in = mk(n_mean), mk(n_halo), mk(n_mean), mk(n_halo)
+        self.one_sided = False        # PutLink.connect: messages are written into / read from the inboxes of the library
 
     def recv_buffers(self):
         return self.mean_in, self.halo_in
@@ -113,24 +152,27 @@ class GpuLevel:
         self.pg.pg3n_set_density(self.h, rho, self.pg.PG_MEM_DEVICE)
 
     def restrict(self):
-        self.pg.pg3n_restrict(self.h, self.mean_out)
-        return self.mean_out, self._token()
+        out = None if self.one_sided else self.mean_out
+        self.pg.pg3n_restrict(self.h, out)
+        return out, self._token()
 
     def absorb(self, t, token):
-        self._after(token)
-        self.pg.pg3n_absorb(self.h, t)
+        if t is not None or self.one_sided:
+            self._after(token)                # one-sided: behind the token's receive (stream-ordered with nccl tokens)
+        self.pg.pg3n_absorb(self.h, t)        # None: this level's MEAN inbox (the token has been received: it is there)
 
     def solve(self):
         self.pg.pg3n_solve(self.h)
 
     def add_exterior(self, t, token):
-        if t is not None:
+        if t is not None or (self.one_sided and self.level > 0):
             self._after(token)
-        self.pg.pg3n_add_exterior(self.h, t)
+        self.pg.pg3n_add_exterior(self.h, t)  # None: level 0, or (one-sided) this level's HALO inbox
 
     def pack_exterior(self):
-        self.pg.pg3n_pack_exterior(self.h, self.halo_out)
-        return self.halo_out, self._token()
+        out = None if self.one_sided else self.halo_out
+        self.pg.pg3n_pack_exterior(self.h, out)
+        return out, self._token()
 
     def potential(self, out):
         self.pg.pg3n_potential(self.h, out, self.pg.PG_MEM_DEVICE)
@@ -148,7 +190,9 @@ class NestedPotential:
     """depth levels of n^3 cells.  world_size 1: all levels on `device`, one stream each.  world_size == depth
     (torch.distributed initialised, backend nccl): this rank owns level `rank` on its own GPU."""
 
-    def __init__(self, n, box0, depth, device=0, dist=None, group=None):
+    def __init__(self, n, box0, depth, device=0, dist=None, group=None, link="put", token_device="cpu"):
+        """link (world_size > 1 only): "put" = one-sided puts into the neighbours' inboxes (PutLink), "sendrecv" =
+        payloads by torch.distributed send / recv (DistLink; needs a backend that moves device tensors, i.e. nccl)."""
         self.n, self.box0, self.depth = n, box0, depth
         world = dist.get_world_size(group) if dist is not None else 1
         if world == 1:
@@ -158,8 +202,10 @@ class NestedPotential:
             if world != depth:
                 raise ValueError(f"one level per rank: world size {world} != depth {depth}")
             self.owned = [dist.get_rank(group)]
-            self.link = DistLink(dist, group)
+            self.link = PutLink(dist, group, token_device) if link == "put" else DistLink(dist, group)
         self.levels = {l: GpuLevel(n, box0, l, depth, device) for l in self.owned}
+        if isinstance(self.link, PutLink):
+            self.link.connect(self.levels[self.owned[0]])
 
     def solve(self, rhos, outs):
         """rhos / outs: {level: device tensor [n][n][n]} for the owned levels.  Enqueues; call synchronize()."""
@@ -177,5 +223,15 @@ class NestedPotential:
         return sum(self.levels[l].pg.pg3n_launch_count(self.levels[l].h) for l in self.owned)
 
     def close(self):
+        if isinstance(self.link, PutLink):
+            # an exported inbox may not be freed while a neighbour still has it open: everybody lets go first
+            for l in self.owned:
+                lev = self.levels[l]
+                if lev.h is not None:
+                    if lev.level > 0:
+                        lev.pg.pg3n_peer_set(lev.h, lev.pg.PG3N_INBOX_MEAN, None)
+                    if lev.level < lev.depth - 1:
+                        lev.pg.pg3n_peer_set(lev.h, lev.pg.PG3N_INBOX_HALO, None)
+            self.link.dist.barrier(group=self.link.group)
         for l in self.owned:
             self.levels[l].close()

@@ -1,6 +1,9 @@
 """Parity of the nested-mesh path (row NEXT-3 of SURVEY.md 8(f): Fig. 8 :306; readings M1-M6)
 against oracle/nested_oracle.py, element by element on seeded densities, level by level, and of each coupling kernel
 against its oracle step.  Bar: rel-L2 <= 1e-10, max pointwise relative <= 1e-9."""
+import os
+import socket
+
 import numpy as np
 import pytest
 
@@ -96,5 +99,96 @@ def test_coupling_kernels_step_by_step_and_call_order_errors():
         check(got_halo, ref_halo, "halo")
         ext1 = out1 - oracle.cart_potential(n, box0 / 2, fine)
         assert np.abs(ext1 - no.prolong(got_halo, n)).max() <= 1e-11 * np.abs(out1).max()
+    finally:
+        pg.pg3n_destroy(h0); pg.pg3n_destroy(h1)
+
+
+# ------------------------------------------------------------------ one level per process, one-sided exchange
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _put_worker(rank, world, port, n, box0, out):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), LOCAL_RANK=str(rank),
+                      WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)       # control messages only: the payload is PUT
+    try:
+        torch.cuda.set_device(0)
+        solver = nested.NestedPotential(n, box0, world, device=0, dist=dist, link="put")
+        try:
+            d_rho = {rank: torch.from_numpy(level_rho(n, rank, world)).cuda()}
+            d_out = {rank: torch.zeros_like(d_rho[rank])}
+            for rep in range(3):                                   # the inboxes are reused safely from solve to solve
+                solver.solve(d_rho, d_out)
+            solver.synchronize()
+            out.put((rank, d_out[rank].cpu().numpy(), solver.launches()))
+        finally:
+            solver.close()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("depth", [2, 3])
+def test_one_level_per_process_one_sided_puts(depth):
+    """The paper's distribution (one nested mesh per image / GPU) with its communication model
+    (one-sided transfers): every level lives in its own PROCESS, exports its inboxes by CUDA IPC handle,
+    and its neighbours' kernels write the level-boundary messages straight into them; torch.distributed (gloo) carries
+    only the one-element tokens.  The processes share the one GPU of this box (no kernel ever waits on another
+    process's kernel: the hand-over is by host messages), so what is exercised is handles, peer pointers, order and
+    reuse of the inboxes -- not NVLink.  Results must equal the oracle."""
+    import torch.multiprocessing as mp
+    n, box0 = 32, 8.0
+    port = _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_put_worker, args=(r, depth, port, n, box0, out)) for r in range(depth)]
+    for p in procs:
+        p.start()
+    got = {}
+    for _ in range(depth):
+        r, phi, launches = out.get(timeout=300)
+        got[r] = phi
+        assert launches > 0
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    ref, _ = no.nested_potential(n, box0, [level_rho(n, l, depth) for l in range(depth)])
+    for l in range(depth):
+        check(got[l], ref[l], f"one-sided, depth {depth}, level {l}")
+
+
+def test_one_sided_inside_one_process_and_inbox_errors():
+    """The same NULL-pointer calls with the neighbour's inbox given by plain device pointer (pg3n_peer_set)."""
+    n, box0 = 32, 4.0
+    rng = np.random.default_rng(12)
+    coarse, fine = rng.random((n, n, n)), rng.random((n, n, n))
+    st = torch.cuda.current_stream().cuda_stream
+    h0 = pg.pg3n_create(n, box0, 0, 2, 0, st)
+    h1 = pg.pg3n_create(n, box0, 1, 2, 0, st)
+    try:
+        for bad in (lambda: pg.pg3n_inbox_export(h1, pg.PG3N_INBOX_MEAN), lambda: pg.pg3n_inbox_export(h0, pg.PG3N_INBOX_HALO)):
+            with pytest.raises(pg.PolargravError) as e:
+                bad()
+            assert e.value.status == pg.PG_ERR_STATE
+        pg.pg3n_set_density(h0, coarse, pg.PG_MEM_HOST)
+        pg.pg3n_set_density(h1, fine, pg.PG_MEM_HOST)
+        with pytest.raises(pg.PolargravError) as e:            # the parent's inbox has not been opened
+            pg.pg3n_restrict(h1, None)
+        assert e.value.status == pg.PG_ERR_STATE
+        handle, mean_addr = pg.pg3n_inbox_export(h0, pg.PG3N_INBOX_MEAN)
+        _, halo_addr = pg.pg3n_inbox_export(h1, pg.PG3N_INBOX_HALO)
+        assert len(handle) == pg.PG_IPC_HANDLE_BYTES and mean_addr % 16 == 0 and halo_addr % 16 == 0
+        pg.pg3n_peer_set(h1, pg.PG3N_INBOX_MEAN, mean_addr)
+        pg.pg3n_peer_set(h0, pg.PG3N_INBOX_HALO, halo_addr)
+        pg.pg3n_restrict(h1, None); pg.pg3n_absorb(h0, None)
+        pg.pg3n_solve(h0); pg.pg3n_solve(h1)
+        pg.pg3n_add_exterior(h0, None); pg.pg3n_pack_exterior(h0, None); pg.pg3n_add_exterior(h1, None)
+        out0 = np.empty((n, n, n)); out1 = np.empty((n, n, n))
+        pg.pg3n_potential(h0, out0, pg.PG_MEM_HOST); pg.pg3n_potential(h1, out1, pg.PG_MEM_HOST)
+        ref, _ = no.nested_potential(n, box0, [coarse, fine])
+        check(out0, ref[0], "level 0"); check(out1, ref[1], "level 1")
     finally:
         pg.pg3n_destroy(h0); pg.pg3n_destroy(h1)
