@@ -214,7 +214,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
+        "config": {"workload": workload_name(cfg) + (f" -- OVERRIDDEN: batch {c.batch} (--batch; not a BASELINE.json workload)" if args.batch else ""),
+                   "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "step": f"O1 direct sum over {len(rings)} of {c.n_r} target rings (bounded sample)"},
         "cells_per_s": value * c.n_r * c.n_phi,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
@@ -263,6 +264,11 @@ def run_ours(args):
 
     cfg = args.config
     c = CONFIGS[cfg]
+    if args.batch:
+        # NOT a BASELINE.json workload: the grid of config `cfg` with `--batch` independent fields per call, so that every
+        # launch runs tens of waves (used for the steady-state ncu capture of profiles/r2_06)
+        import dataclasses
+        c = dataclasses.replace(c, batch=args.batch)
     field_bytes = 8 * c.n_r * c.n_phi
     pair_bytes = 2 * field_bytes * c.batch
     R = int(min(64, max(4, -(-4 * L2_BYTES // pair_bytes))))
@@ -362,7 +368,7 @@ def run_ours(args):
     per_launch_ms = [kms[i] / max(1, kn[i]) for i in range(pg.PG_NUM_KERNELS)]
     dom = int(np.argmax(per_launch_ms))
     peak, peak_src = load_peaks()
-    ncu, ncu_why = ncu_record(cfg)
+    ncu, ncu_why = ncu_record(cfg) if not args.batch else (None, "--batch overrides the config the ncu record was captured at")
     kbytes = [pg.pg_kernel_algorithmic_bytes(h, i, c.batch) for i in range(pg.PG_NUM_KERNELS)]
     achieved = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
     path_bytes = pg.pg_algorithmic_bytes(h, c.batch)
@@ -420,7 +426,8 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
+        "config": {"workload": workload_name(cfg) + (f" -- OVERRIDDEN: batch {c.batch} (--batch; not a BASELINE.json workload)" if args.batch else ""),
+                   "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
                    "parallelism": "replicas only (no collective)" if world > 1 else "single GPU",
                    "path": ("one cooperative launch per solve (fused_solve_kernel: a2 | grid barrier | a3+a4r | grid barrier | a4phi)"
                             if fused else "three launches per solve (rows_fwd, cols, rows_inv) chained by programmatic dependent launch"),
@@ -944,6 +951,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
     ap.add_argument("--nested", type=int, default=0, help="D nested 3-D mesh levels of --cart N cells per edge (row NEXT-3; default N = 64); under torchrun with WORLD_SIZE = D one level per GPU")
+    ap.add_argument("--batch", type=int, default=0, help="override the config's batch (fields per call); not a BASELINE.json workload")
     ap.add_argument("--nested-link", default="put", choices=["put", "sendrecv"],
                     help="--nested under torchrun: one-sided puts into the neighbours' inboxes (default) or NCCL send / recv of the messages")
     ap.add_argument("--no-fused", action="store_true", help="small grids: force the three-kernel path (PG_OPT_FUSED = 0)")
