@@ -181,6 +181,10 @@ pg_status pg_set_stream(pg_solver *s, void *cuda_stream);
  *       three launches, as long as the batch is small enough for all its CTAs to be resident at once: such solves are
  *       bound by the host's launch rate, not by the GPU.  Same arithmetic, bit-identical results.  0 forces the
  *       three-kernel path (which pg_profile passes, pg_acceleration and non-symmetric softening always take).
+ *       Trade-off: the fused launch is what makes several small solves in flight (PG_OPT_LANES, host-staged pipelines)
+ *       cheap -- one launch each -- but ONE solve takes longer in it (two grid-wide barriers: 9.6 / 13.9 / 16.3 us at
+ *       64^2 / 256^2 / 512^2) than in three kernels chained by programmatic dependent launch once the launch queue is
+ *       full (8.5 / 8.7 / 10.2 us); a long time series of DEPENDENT small solves on one stream may prefer 0.
  * Returns PG_ERR_INVALID_ARG for an unknown option or value. */
 typedef enum { PG_OPT_DENSITY_STABLE = 1, PG_OPT_LANES = 2, PG_OPT_FUSED = 3 } pg_option;
 pg_status pg_set_option(pg_solver *s, pg_option option, int value);
