@@ -347,9 +347,10 @@ def test_fused_single_launch_equals_three_kernels_bit_for_bit(n_r, n_phi, batch)
         s.close()
 
 
-def test_fused_solves_on_four_lanes_equal_the_ordinary_path():
-    """Small grids in throughput mode: PG_OPT_LANES = 4 deals the fused launches out over four internal streams."""
-    n_r = n_phi = 256
+@pytest.mark.parametrize("n_r,n_phi", [(64, 64), (256, 256), (512, 512)])
+def test_fused_solves_on_four_lanes_equal_the_ordinary_path(n_r, n_phi):
+    """Small grids in throughput mode, the launch configuration bench.py times for configs 1-3: PG_OPT_LANES = 4 deals
+    the fused launches out over four internal streams; results equal the one-lane three-kernel path bit for bit."""
     st = torch.cuda.Stream()
     s = pg.Solver(n_r, n_phi, 1.0, 500.0, 0.01, device=0, cuda_stream=st.cuda_stream)
     try:
