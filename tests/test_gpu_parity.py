@@ -353,7 +353,7 @@ def test_partial_batch_uses_the_first_fields_only():
 
 
 @pytest.mark.parametrize("n_r,n_phi,batch", [(64, 64, 1), (256, 128, 2), (32, 512, 1), (512, 256, 3), (1024, 64, 1),
-                                             (64, 2048, 1), (2048, 32, 1), (1024, 1024, 2)])
+                                             (64, 2048, 1), (2048, 32, 1), (1024, 1024, 2), (2048, 2048, 1)])
 def test_repeated_solves_are_bitwise_reproducible(n_r, n_phi, batch):
     """compute-sanitizer is closed on the GPU pool, so shared-memory hazards (the passes exchange through
     shared memory under named barriers and mbarriers) are hunted this way: 12 repeats of the same solve,
