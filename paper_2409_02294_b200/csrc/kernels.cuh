@@ -23,10 +23,17 @@
 #define PG_ROW_THREADS 128
 #endif
 #ifndef PG_ROW_THREADS_BIG
-#define PG_ROW_THREADS_BIG 256      // n_phi >= 2048: 4 rows per CTA (64-byte runs in W), two CTAs per SM.  W is stored
-                                    // transposed, so a CTA of ROWS rows touches it in runs of ROWS * 16 bytes, and the L2
-                                    // serves 32-byte runs at half the rate of 64-byte ones (4.0 against 5.3 (stores) ..
-                                    // 7.7 TB/s (loads), measured): with 2 rows per CTA the row kernels were bound by it.
+#define PG_ROW_THREADS_BIG 256      // n_phi >= 2048, forward row kernel: 4 rows per CTA (64-byte runs in W), two CTAs per
+                                    // SM.  W is stored transposed, so a CTA of ROWS rows touches it in runs of ROWS * 16
+                                    // bytes, and the L2 serves 32-byte runs at half the rate of 64-byte ones (4.0 against
+                                    // 5.3 (stores) .. 7.7 TB/s (loads), measured): with 2 rows per CTA the kernel's
+                                    // transposed STORES were bound by it.
+#endif
+#ifndef PG_ROW_THREADS_BIG_INV
+#define PG_ROW_THREADS_BIG_INV 128  // n_phi >= 2048, inverse row kernel: 2 rows per CTA, FOUR CTAs per SM.  Its transposed
+                                    // READS are one TMA tile per item (asynchronous, off the LSU), so the run length
+                                    // matters less than the number of independent items an SM has in flight: 12.47 us
+                                    // (4 rows, 2 CTAs) -> 11.57 us (2 rows, 4 CTAs) per 2048^2 field at saturation.
 #endif
 #ifndef PG_ROW_INLINE_FROM
 #define PG_ROW_INLINE_FROM 2048     // from this n_phi on the row kernels stage their input INSIDE the rows' own lines
@@ -39,10 +46,10 @@ namespace pgk {
 
 // ---------------------------------------------------------------- shapes
 // rows per CTA in the phi passes: W is written/read in runs of ROWS*16 bytes
-__host__ __device__ constexpr int rows_per_cta(int nphi)
+__host__ __device__ constexpr int rows_per_cta(int nphi, bool inverse = false)
 {
     const int T = nphi / 32;
-    const int r = (nphi >= 2048 ? PG_ROW_THREADS_BIG : PG_ROW_THREADS) / (T > 0 ? T : 1);
+    const int r = (nphi >= 2048 ? (inverse ? PG_ROW_THREADS_BIG_INV : PG_ROW_THREADS_BIG) : PG_ROW_THREADS) / (T > 0 ? T : 1);
     return r < 2 ? 2 : (r > 16 ? 16 : r);
 }
 // azimuthal modes per CTA in the r pass
@@ -55,12 +62,13 @@ __host__ __device__ constexpr int modes_per_cta(int nr)
 // Shared-memory slots between the lines of two rows of a CTA.  In the row-fastest pass a
 // quarter-warp touches (8 rows) or (4 rows x 2 neighbouring 9-slot blocks): STRIDE = 1 (mod 8)
 // resp. 2 (mod 8) spreads them over the eight 16-byte bank groups.
-template <int NPHI>
+// INV: the shape of the inverse row kernel (it differs from the forward kernel's only at n_phi >= 2048, see above)
+template <int NPHI, bool INV = false>
 struct RowShape {
     static constexpr int L = NPHI / 2;
     typedef Plan<L, ROW> P;
     static constexpr int T = P::T;
-    static constexpr int ROWS = rows_per_cta(NPHI);
+    static constexpr int ROWS = rows_per_cta(NPHI, INV);
     static constexpr int SKEW = (ROWS >= 8) ? 1 : (8 / ROWS);
     static constexpr int STRIDE = ((P::LINE + 7) / 8) * 8 + SKEW;   // slots per row line
     static constexpr int THREADS = ROWS * T;
@@ -467,7 +475,7 @@ __device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double
                                               const long w_field_stride, const long phi_field_stride, const int block,
                                               const int nblocks, unsigned char *smem_raw, const CUtensorMap *tmap)
 {
-    typedef RowShape<NPHI> S;
+    typedef RowShape<NPHI, true> S;
     typedef Plan<S::L, ROW> P;
     constexpr int L = S::L, T = S::T, ROWS = S::ROWS;
     cplx *smem = reinterpret_cast<cplx *>(smem_raw);
@@ -583,7 +591,7 @@ __device__ __forceinline__ void rows_inv_body(const cplx *__restrict__ W, double
     }
 }
 template <int NPHI, bool HALF = false>
-__global__ void __launch_bounds__(RowShape<NPHI>::THREADS, RowShape<NPHI>::MIN_CTAS)
+__global__ void __launch_bounds__(RowShape<NPHI, true>::THREADS, RowShape<NPHI, true>::MIN_CTAS)
 rows_inv_kernel(const cplx *__restrict__ W, double *__restrict__ phi, const cplx *__restrict__ tw,
                 const double *__restrict__ oscale, const int n_rows, const int n_items, const long w_field_stride,
                 const long phi_field_stride, const __grid_constant__ CUtensorMap tmap)
@@ -714,6 +722,7 @@ template <int NR, int NPHI>
 struct FusedShape {
     typedef RowShape<NPHI> RS;
     typedef ColShape<NR> CS;
+    static_assert(RowShape<NPHI, true>::ROWS == RS::ROWS && RowShape<NPHI, true>::SMEM == RS::SMEM, "one row shape below 2048");
     static_assert(!RS::INLINE && NPHI >= 64 && NPHI <= 512 && NR >= 64 && NR <= 512, "fused path: 64 .. 512 per axis");
     static constexpr int THREADS = RS::THREADS > CS::THREADS ? RS::THREADS : CS::THREADS;
     static constexpr size_t SMEM = RS::SMEM > CS::SMEM ? RS::SMEM : CS::SMEM;

@@ -40,7 +40,7 @@ struct Events4 { cudaEvent_t e[4]; };
 struct pg_solver {
     int n_r = 0, n_phi = 0, max_batch = 1, device = 0;
     double r_in = 0, r_out = 0, eps = 0, du = 0, dphi = 0;
-    int sm_count = 0, row_ctas = 0;   // persistent grid of the row kernels
+    int sm_count = 0, row_ctas = 0, row_ctas_inv = 0;   // persistent grids of the forward / inverse row kernel
     // small grids (64 .. 512 per axis): the whole solve in one cooperative launch (kernels.cuh, fused_solve_kernel)
     // tensor maps of the W buffers rows_inv_kernel reads as 4-D TMA tiles (n_phi >= PG_ROW_INLINE_FROM), by buffer
     struct RowTmap { const void *base; int n_rows, fields; long stride; CUtensorMap map; };
@@ -288,7 +288,7 @@ pg_status launch_rows_fwd(pg_solver *s, const double *sigma, cplx *Z, const doub
 template <int NPHI>
 pg_status row_tmap(pg_solver *s, const cplx *Z, int n_rows, int fields, long z_stride, CUtensorMap *out)
 {
-    typedef pgk::RowShape<NPHI> S;
+    typedef pgk::RowShape<NPHI, true> S;
     typedef pgk::Plan<S::L, pgk::ROW> P;
     memset(out, 0, sizeof *out);
     if constexpr (!S::TILE) {
@@ -329,9 +329,9 @@ template <int NPHI>
 pg_status launch_rows_inv(pg_solver *s, const cplx *Z, double *phi, int batch, long z_stride, long phi_stride,
                           cudaStream_t st, const double *oscale)
 {
-    typedef pgk::RowShape<NPHI> S;
+    typedef pgk::RowShape<NPHI, true> S;
     const int n_items = (s->n_r / S::ROWS) * batch;
-    const int grid = n_items < s->row_ctas ? n_items : s->row_ctas;
+    const int grid = n_items < s->row_ctas_inv ? n_items : s->row_ctas_inv;
     CUtensorMap tmap;
     pg_status rc = row_tmap<NPHI>(s, Z, s->n_r, batch, z_stride, &tmap);
     if (rc != PG_OK) return rc;
@@ -464,16 +464,17 @@ template <int NPHI>
 pg_status prepare_rows(pg_solver *s)
 {
     typedef pgk::RowShape<NPHI> S;
+    typedef pgk::RowShape<NPHI, true> SI;
     PG_CUDA(s, cudaFuncSetAttribute(pgk::rows_fwd_kernel<NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)S::SMEM));
     PG_CUDA(s, cudaFuncSetAttribute(pgk::rows_inv_kernel<NPHI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)S::SMEM));
-    // persistent grid: as many CTAs as are resident at once (the smaller of the two kernels' occupancies)
+                                    (int)SI::SMEM));
+    // persistent grids: as many CTAs as are resident at once
     int occ_f = 0, occ_i = 0;
     PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, pgk::rows_fwd_kernel<NPHI>, S::THREADS, S::SMEM));
-    PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, pgk::rows_inv_kernel<NPHI>, S::THREADS, S::SMEM));
-    const int occ = occ_f < occ_i ? occ_f : occ_i;
-    s->row_ctas = (occ > 0 ? occ : 1) * s->sm_count;
+    PG_CUDA(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, pgk::rows_inv_kernel<NPHI>, SI::THREADS, SI::SMEM));
+    s->row_ctas = (occ_f > 0 ? occ_f : 1) * s->sm_count;
+    s->row_ctas_inv = (occ_i > 0 ? occ_i : 1) * s->sm_count;
     return PG_OK;
 }
 template <int NR>
@@ -1493,7 +1494,10 @@ pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
     pgk::ycols_inv_kernel<N><<<ygrid, Y::THREADS, Y::SMEM, st>>>(s->d_Yt, in->d_W, in->d_tw_col);
     in->launches++;
     // inverse x pass, cropped to the first N reals of every row: Phi[z][y][x]
-    PG3_CUDA(s, launch_pdl(pgk::rows_inv_kernel<M, true>, dim3(rgrid), dim3(RS::THREADS), RS::SMEM, st, (const cplx *)in->d_W,
+    typedef pgk::RowShape<M, true> RSI;
+    static_assert(RSI::ROWS == RS::ROWS && RSI::SMEM == RS::SMEM, "one row shape below 2048");
+    const int rgrid_inv = n_items < in->row_ctas_inv ? n_items : in->row_ctas_inv;
+    PG3_CUDA(s, launch_pdl(pgk::rows_inv_kernel<M, true>, dim3(rgrid_inv), dim3(RSI::THREADS), RSI::SMEM, st, (const cplx *)in->d_W,
                            d_phi, (const cplx *)in->d_tw_row, (const double *)s->d_ones, N, n_items, ws, (long)N * N, CUtensorMap{}));
     in->launches++;
     PG3_CUDA(s, cudaGetLastError());
