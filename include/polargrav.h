@@ -145,6 +145,49 @@ pg_status pg_acceleration(pg_solver *s, double *a_r, double *a_phi, int batch, p
 /* pg_destroy -- frees everything the solver owns. pg_destroy(NULL) is a no-op returning PG_OK. */
 pg_status pg_destroy(pg_solver *s);
 
+/* ---------------------------------------------------------------- the one call that never allocates
+ * pg_potential_direct_static -- the direct summation of pg_potential_direct (row a5; same kernels, same grid
+ * conventions, symmetric softening, G = 1) for ONE field, with no solver object and no allocation of any kind.
+ *
+ * Who it is for.  Everything else in this header starts from pg_create*, which takes device memory (tables, the
+ * spectrum, workspaces -- and pg_potential may add more on first use: a second workspace under
+ * PG_OPT_DENSITY_STABLE, one pair per lane, staging buffers for host memspaces).  Some programs cannot give it any:
+ *   - a simulation that sized its own arena (or a framework's caching allocator) to take all free HBM at start-up:
+ *     a cudaMalloc issued later simply fails;
+ *   - a job held to a fixed device-memory budget (a MIG slice or an MPS limit sized to the application);
+ *   - a plug-in or callback that is handed device pointers by its host program and has no licence to create
+ *     device buffers of its own.
+ * Such a caller can still cross-check a potential it holds, or solve a small grid outright (the sum costs
+ * (n_r n_phi)^2 pair terms: microseconds at 64^2, about a second at 2048^2), by passing its own two arrays.
+ *
+ * How.  Beyond Sigma and Phi the kernel reads three grid tables (r_i, dA_i, sin^2(pi l / n_phi)).  For this call
+ * they live in a fixed array inside the library image: 3 * PG_STATIC_MAX_N doubles = 48 KiB, present on every GPU
+ * that loads the library until the process exits, whether or not the call is ever made.  The tables are computed
+ * on the host exactly as pg_create* computes them and sent to that array on `cuda_stream` ahead of the kernel, so
+ * the result equals pg_potential_direct's for the same grid.  The call uses no cudaMalloc, cudaFree,
+ * cudaHostAlloc or other allocating routine, and creates no stream or event.
+ *
+ *   sigma, phi   device pointers on `device`, [n_r][n_phi], 16-byte aligned, not overlapping; borrowed for the
+ *                duration of the enqueued work.
+ *   n_r, n_phi   powers of two in [PG_MIN_N, PG_STATIC_MAX_N]; anything larger does not fit the fixed array and is
+ *                refused with PG_ERR_UNSUPPORTED (the text names the limit).  r_in, r_out, eps as in pg_create.
+ *   device       CUDA device ordinal, or -1 for the current device.  cuda_stream: borrowed, NULL = default stream.
+ * Returns after enqueue; the tables leave from ordinary (pageable) host memory, so the host may first wait for
+ * work already on the stream.  Errors: the status, with the text in pg_last_error(NULL).
+ *
+ * One-time set-up.  The first call on each device asks the runtime for the device address of the fixed array
+ * (cudaGetSymbolAddress, with that device current) and checks the device is sm_100.  Make that first call before
+ * any stream capture is begun.
+ *
+ * Sharing.  There is ONE array per GPU, used by every call from every thread and stream, and it keeps whatever the
+ * last call wrote.  Nothing in it has to start at zero: each call rewrites every entry its kernel will read.
+ * Calls on the same stream are ordered and safe.  Calls whose GPU work may overlap -- different streams with no
+ * event between them, different host threads -- race on the tables: one call's upload can land under the other's
+ * running kernel.  Order them (one stream, or an event from each call to the next). */
+#define PG_STATIC_MAX_N 2048
+pg_status pg_potential_direct_static(const double *sigma, double *phi, int n_r, int n_phi, double r_in,
+                                     double r_out, double eps, int device, void *cuda_stream);
+
 /* ---------------------------------------------------------------- helpers */
 
 /* Grid tables (host pointers, any may be NULL): r[n_r] cell-centre radii, phi[n_phi] cell-centre

@@ -18,6 +18,7 @@ PG_OK = 0
 PG_ERR_INVALID_ARG, PG_ERR_UNSUPPORTED, PG_ERR_CUDA, PG_ERR_NOMEM, PG_ERR_STATE = -1, -2, -3, -4, -5
 PG_MEM_HOST, PG_MEM_HOST_PINNED, PG_MEM_DEVICE = 0, 1, 2
 PG_NUM_KERNELS = 3
+PG_STATIC_MAX_N = 2048      # largest grid axis of pg_potential_direct_static (its tables are a fixed array)
 PG_OPT_DENSITY_STABLE = 1
 PG_OPT_LANES = 2
 PG_OPT_FUSED = 3
@@ -30,7 +31,7 @@ EXPORTS = (
     "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_set_option", "pg_synchronize",
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
-    "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush",
+    "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush", "pg_potential_direct_static",
     "pg3_create", "pg3_set_density", "pg3_potential", "pg3_synchronize", "pg3_destroy", "pg3_launch_count",
     "pg3_algorithmic_bytes", "pg3_last_error",
     "pg3n_create", "pg3n_set_density", "pg3n_restrict", "pg3n_absorb", "pg3n_solve", "pg3n_add_exterior",
@@ -66,6 +67,7 @@ def lib():
         L.pg_set_softening.argtypes = [vp, i]
         L.pg_acceleration.argtypes = [vp, vp, vp, i, i]
         L.pg_destroy.argtypes = [vp]
+        L.pg_potential_direct_static.argtypes = [vp, vp, i, i, d, d, d, i, vp]
         L.pg_grid.argtypes = [vp, vp, vp, vp]
         L.pg_set_stream.argtypes = [vp, vp]
         L.pg_set_option.argtypes = [vp, i, i]
@@ -182,6 +184,13 @@ def pg_acceleration(h, a_r, a_phi, batch, where):
 
 def pg_destroy(h):
     _check(lib().pg_destroy(h))
+
+
+def pg_potential_direct_static(sigma, phi, n_r, n_phi, r_in, r_out, eps, device=-1, cuda_stream=None):
+    """Direct summation of one field with no solver and no allocation (tables in a fixed 48 KiB array of the library);
+    sigma, phi: device arrays.  Errors carry the text of pg_last_error(NULL)."""
+    _check(lib().pg_potential_direct_static(_ptr(sigma), _ptr(phi), n_r, n_phi, r_in, r_out, eps, device,
+                                            ctypes.c_void_p(cuda_stream) if cuda_stream else None))
 
 
 def pg_grid(h, n_r, n_phi):

@@ -1955,3 +1955,127 @@ long pg3n_launch_count(const pg3n_level *s) { return s ? s->launches : 0; }
 const char *pg3n_last_error(const pg3n_level *s) { return s ? s->err : g_create_error; }
 
 }  // extern "C"
+
+// =================================================================== the one call that never allocates
+// pg_potential_direct_static (polargrav.h): direct summation for callers that cannot obtain device memory -- their
+// program gave all of it to its own arena at start-up, runs inside a fixed memory budget, or only lends them pointers.
+// The three grid tables the direct kernels read (r, dA, s2: the only global memory they touch besides Sigma and Phi,
+// cudaMalloc'ed by create_impl on the ordinary path) sit here in a fixed array of the library image instead:
+// 3 * PG_STATIC_MAX_N doubles = 48 KiB per GPU that loads the library, held until the process exits.
+//
+// The name below is only a stand-in on the host side: host code may not pass it to a kernel or a copy as if it were a
+// device address.  static_tables_address() obtains the real address once per device, with that device current, and
+// everything on the host goes through that pointer.
+static __device__ __align__(256) double g_static_tables[3 * PG_STATIC_MAX_N];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+double *g_static_tables_on[kStaticMaxDevices] = {};   // device address of g_static_tables, by device ordinal
+
+// One-time set-up per device.  `device` must be the current device (the caller holds a DeviceGuard).
+pg_status static_tables_address(int device, double **out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_tables_on[device]) {
+        int major = 0;
+        PG_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+        if (major != 10) {
+            set_err(nullptr, "device %d is not sm_100; this library is built for sm_100a (B200) only and has no fallback", device);
+            return PG_ERR_UNSUPPORTED;
+        }
+        double *p = nullptr;
+        PG_CUDA(nullptr, cudaGetSymbolAddress((void **)&p, g_static_tables));
+        if (!p) { set_err(nullptr, "cudaGetSymbolAddress returned a null address for the static tables"); return PG_ERR_CUDA; }
+        g_static_tables_on[device] = p;
+    }
+    *out = g_static_tables_on[device];
+    return PG_OK;
+}
+
+}  // namespace
+
+extern "C" pg_status pg_potential_direct_static(const double *sigma, double *phi, int n_r, int n_phi, double r_in,
+                                                double r_out, double eps, int device, void *cuda_stream)
+{
+    g_create_error[0] = 0;
+    // host-side checks first: none of them needs a device
+    if (!sigma || !phi) { set_err(nullptr, "pg_potential_direct_static: sigma or phi is NULL"); return PG_ERR_INVALID_ARG; }
+    if (!(r_in > 0.0) || !(r_out > r_in) || !(eps > 0.0) || !std::isfinite(r_out) || !std::isfinite(eps)) {
+        set_err(nullptr, "pg_potential_direct_static: need 0 < r_in < r_out and eps > 0");
+        return PG_ERR_INVALID_ARG;
+    }
+    if (n_r > PG_STATIC_MAX_N || n_phi > PG_STATIC_MAX_N) {
+        set_err(nullptr, "pg_potential_direct_static: grid %dx%d does not fit the fixed table array (at most %d cells per "
+                         "axis); this call cannot allocate a larger one -- use pg_create + pg_potential_direct",
+                n_r, n_phi, PG_STATIC_MAX_N);
+        return PG_ERR_UNSUPPORTED;
+    }
+    if (!is_pow2(n_r) || !is_pow2(n_phi) || n_r < PG_MIN_N || n_phi < PG_MIN_N) {
+        set_err(nullptr, "pg_potential_direct_static: unsupported grid %dx%d: n_r and n_phi must be powers of two in [%d, %d]",
+                n_r, n_phi, PG_MIN_N, PG_STATIC_MAX_N);
+        return PG_ERR_UNSUPPORTED;
+    }
+    const size_t fbytes = (size_t)n_r * n_phi * sizeof(double);
+    if ((((uintptr_t)sigma | (uintptr_t)phi) & 15u) != 0) {
+        set_err(nullptr, "pg_potential_direct_static: sigma and phi must be 16-byte aligned device pointers");
+        return PG_ERR_INVALID_ARG;
+    }
+    if (ranges_overlap(sigma, fbytes, phi, fbytes)) {
+        set_err(nullptr, "pg_potential_direct_static: phi overlaps sigma");
+        return PG_ERR_INVALID_ARG;
+    }
+    int ndev = 0;
+    PG_CUDA(nullptr, cudaGetDeviceCount(&ndev));
+    if (device < 0) PG_CUDA(nullptr, cudaGetDevice(&device));
+    if (device >= ndev || device >= kStaticMaxDevices) {
+        set_err(nullptr, "pg_potential_direct_static: device %d out of range (%d devices)", device, ndev);
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(device);          // current for the set-up, the copy and the launch; restored on return
+    double *tables = nullptr;
+    pg_status st = static_tables_address(device, &tables);
+    if (st != PG_OK) return st;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    // the tables of create_impl (readings A1, A2), packed [r | dA | s2]; every entry the kernel reads is rewritten
+    double host[3 * PG_STATIC_MAX_N];
+    double *h_r = host, *h_dA = host + n_r, *h_s2 = host + 2 * n_r;
+    {
+        const long double du = logl((long double)r_out / (long double)r_in) / n_r;
+        const long double dphi = 2.0L * kPiL / n_phi;
+        for (int i = 0; i < n_r; ++i) {
+            const long double ri = (long double)r_in * expl(((long double)i + 0.5L) * du);
+            h_r[i] = (double)ri;
+            h_dA[i] = (double)(ri * ri * sinhl(du) * dphi);
+        }
+        for (int j = 0; j < n_phi; ++j) {
+            const long double sn = sinl(kPiL * j / n_phi);
+            h_s2[j] = (double)(sn * sn);
+        }
+    }
+    // pageable source: the runtime has taken its copy of `host` when this returns
+    PG_CUDA(nullptr, cudaMemcpyAsync(tables, host, (size_t)(2 * n_r + n_phi) * sizeof(double), cudaMemcpyHostToDevice, stream));
+    const double *d_r = tables, *d_dA = tables + n_r, *d_s2 = tables + 2 * n_r;
+
+    // same shapes as launch_direct
+    const double eps2 = eps * eps;
+    const long fs = (long)n_r * n_phi;
+    const dim3 grid(n_r, 1);
+    if (n_phi >= 256) {
+        const int R = n_phi >= 1024 ? 16 : 8;
+        const size_t smem = ((size_t)n_phi + (size_t)(2 * n_phi / R) * (R + 2)) * sizeof(double);
+        if (R == 16) {
+            PG_CUDA(nullptr, cudaFuncSetAttribute(pgk::direct_tiled_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            pgk::direct_tiled_kernel<16><<<grid, n_phi / 16, smem, stream>>>(sigma, phi, d_r, d_dA, d_s2, n_r, n_phi, eps2, 0, fs, fs);
+        } else {
+            pgk::direct_tiled_kernel<8><<<grid, n_phi / 8, smem, stream>>>(sigma, phi, d_r, d_dA, d_s2, n_r, n_phi, eps2, 0, fs, fs);
+        }
+    } else {
+        const size_t smem = 2 * (size_t)n_phi * sizeof(double);
+        pgk::direct_kernel<1><<<grid, n_phi, smem, stream>>>(sigma, phi, d_r, d_dA, d_s2, n_r, n_phi, eps2, 0, fs, fs);
+    }
+    PG_CUDA(nullptr, cudaGetLastError());
+    return PG_OK;
+}
