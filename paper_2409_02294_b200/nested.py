@@ -61,9 +61,11 @@ class PutLink:
     """One level per rank, one-sided: the payload has been PUT into the receiver's inbox by the sender's kernel; send /
     recv move a one-element token that tells the receiver so.  `connect` exchanges the IPC handles once."""
 
-    def __init__(self, dist, group=None, token_device="cpu"):
+    def __init__(self, dist, group=None, token_device=None):
         import torch
         self.dist, self.group = dist, group
+        if token_device is None:       # an NCCL group moves device tensors only, a gloo group host tensors
+            token_device = "cuda" if str(dist.get_backend(group)).lower() == "nccl" else "cpu"
         self.tok = torch.zeros(1, dtype=torch.int32, device=token_device)
 
     def connect(self, level):
@@ -190,7 +192,7 @@ class NestedPotential:
     """depth levels of n^3 cells.  world_size 1: all levels on `device`, one stream each.  world_size == depth
     (torch.distributed initialised, backend nccl): this rank owns level `rank` on its own GPU."""
 
-    def __init__(self, n, box0, depth, device=0, dist=None, group=None, link="put", token_device="cpu"):
+    def __init__(self, n, box0, depth, device=0, dist=None, group=None, link="put", token_device=None):
         """link (world_size > 1 only): "put" = one-sided puts into the neighbours' inboxes (PutLink), "sendrecv" =
         payloads by torch.distributed send / recv (DistLink; needs a backend that moves device tensors, i.e. nccl)."""
         self.n, self.box0, self.depth = n, box0, depth
@@ -202,6 +204,8 @@ class NestedPotential:
             if world != depth:
                 raise ValueError(f"one level per rank: world size {world} != depth {depth}")
             self.owned = [dist.get_rank(group)]
+            if token_device is None and str(dist.get_backend(group)).lower() == "nccl":
+                token_device = f"cuda:{device}"       # the level's own GPU; PutLink picks "cpu" for gloo
             self.link = PutLink(dist, group, token_device) if link == "put" else DistLink(dist, group)
         self.levels = {l: GpuLevel(n, box0, l, depth, device) for l in self.owned}
         if isinstance(self.link, PutLink):

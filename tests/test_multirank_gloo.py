@@ -164,3 +164,35 @@ def test_nested_levels_one_per_rank_world2_gloo():
     for l in range(world):
         assert np.array_equal(levels[l].phi, ref[l])
     assert nested.message_counts(8) == (64, 216)
+
+
+def _putlink_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), LOCAL_RANK=str(rank),
+                      WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        link = nested.PutLink(dist)               # no token_device given: taken from the group's backend
+        if rank == 0:
+            link.tok.fill_(41)
+            link.send(0, 1, None)
+        else:
+            link.recv(0, 1)
+        out.put((rank, str(link.tok.device), int(link.tok.item())))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_putlink_token_device_follows_the_backend_world2_gloo():
+    """PutLink's one-element token must live where the group's backend can move it: host memory for gloo (device memory
+    for nccl -- the default used to be "cpu" whatever the backend, which an NCCL-only group cannot send)."""
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_putlink_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = dict((r, (dev, val)) for r, dev, val in (out.get(timeout=120) for _ in range(world)))
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    assert got[0][0] == "cpu" and got[1] == ("cpu", 41)
