@@ -381,6 +381,9 @@ pg_status launch_fused(pg_solver *s, const double *sigma, double *phi, cplx *W, 
     PG_CUDA(s, cudaLaunchCooperativeKernel((const void *)pgk::fused_solve_kernel<NR, NPHI>, dim3(grid), dim3(F::THREADS), args,
                                            F::SMEM, st));
     s->launches++;
+    // an ordinary (non-PDL-releasing) kernel: everything before it on the stream, including the output range an earlier
+    // rows_inv_kernel recorded, is complete before any kernel behind it starts
+    forget_early_release_output(s->device, st);
     return PG_OK;
 }
 #define PG_FUSED_DISPATCH_PHI(NR, CALL)                         \
@@ -685,8 +688,10 @@ pg_status ensure_pinned(pg_solver *s, bool in, bool out)
 pg_status drain_profile(pg_solver *s)
 {
     if (s->prof_used == 0) return PG_OK;
+    const int used = s->prof_used;
+    s->prof_used = 0;          // whatever happens below, the slots are free again: one failure must not fail every later call
     PG_CUDA(s, cudaStreamSynchronize(s->stream));
-    for (int c = 0; c < s->prof_used; ++c) {
+    for (int c = 0; c < used; ++c) {
         for (int k = 0; k < PG_NUM_KERNELS; ++k) {
             float ms = 0.f;
             PG_CUDA(s, cudaEventElapsedTime(&ms, s->prof_pool[c].e[k], s->prof_pool[c].e[k + 1]));
@@ -694,14 +699,23 @@ pg_status drain_profile(pg_solver *s)
             s->prof_n[k] += 1;
         }
     }
-    s->prof_used = 0;
     return PG_OK;
 }
 
-// the three kernels of one solve of `batch` fields starting at the given pointers
-pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx *d_W, int batch)
+// the three kernels of one solve of `batch` fields starting at the given pointers.  allow_lanes: the solve may go to
+// a lane stream (PG_OPT_LANES) -- only the all-resident call site of potential_common says so; the staged host
+// pipeline orders its copies against the solver's stream and must stay on it (polargrav.h: host memspaces keep
+// using the solver's stream)
+pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx *d_W, int batch, bool allow_lanes)
 {
     const long fs = (long)s->field, ws = (long)(s->half + 1) * s->n_r;
+    if (s->soft != PG_SOFT_SYMMETRIC) {
+        // field / source softening: complex spectrum, variants.cuh.  No per-kernel profiling on this path, so no
+        // profiling slot is taken for it (a slot with unrecorded events would poison drain_profile).
+        const int kind = 0;
+        double *out = d_phi;
+        return solve_variant(s, d_sigma, d_W, batch, 1, &kind, &out);
+    }
     Events4 *ev = nullptr;
     if (s->profile) {
         if (s->prof_used == kMaxProfiledCalls) {
@@ -716,13 +730,7 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
         ev = &s->prof_pool[s->prof_used++];
         PG_CUDA(s, cudaEventRecord(ev->e[0], s->stream));
     }
-    if (s->soft != PG_SOFT_SYMMETRIC) {
-        // field / source softening: complex spectrum, variants.cuh (no per-kernel profiling on this path)
-        const int kind = 0;
-        double *out = d_phi;
-        return solve_variant(s, d_sigma, d_W, batch, 1, &kind, &out);
-    }
-    if (s->lanes >= 2 && s->density_stable && !s->sigma_from_host && !ev && d_W == s->d_W) {
+    if (allow_lanes && s->lanes >= 2 && s->density_stable && !s->sigma_from_host && !ev && d_W == s->d_W) {
         // two solves in flight: this one goes to the lane the previous one did not take.  The caller has promised
         // (polargrav.h, PG_OPT_LANES) that density and potential are touched by nothing else in flight.
         const int L = s->lane_next;
@@ -1110,7 +1118,7 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
     if (!host_out && !s->sigma_from_host) {
         // everything resident: one batched launch per kernel
         if (direct) return launch_direct(s, s->d_sigma, phi, rings ? ring0 : 0, rings ? n_rings : s->n_r, batch);
-        return solve_fields(s, s->d_sigma, phi, s->d_W, batch);
+        return solve_fields(s, s->d_sigma, phi, s->d_W, batch, true);
     }
 
     // staged pipeline: field b is solved as soon as its H2D copy has landed, and copied back
@@ -1127,7 +1135,7 @@ static pg_status potential_common(pg_solver *s, double *phi, int batch, pg_memsp
         const double *sg = s->d_sigma + (size_t)b * s->field;
         double *dst = host_out ? d_out + (size_t)b * s->field : phi + (size_t)b * out_field;
         if (direct) st = launch_direct(s, sg, dst, rings ? ring0 : 0, rings ? n_rings : s->n_r, 1);
-        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * (s->half + 1) * s->n_r, 1);
+        else st = solve_fields(s, sg, dst, s->d_W + (size_t)b * (s->half + 1) * s->n_r, 1, false);
         if (st != PG_OK) return st;
         if (host_out) {
             PG_CUDA(s, cudaEventRecord(s->ev_solved[b], s->stream));
@@ -1500,6 +1508,9 @@ pg_status cart_solve(pg3_solver *s, const double *d_rho, double *d_phi)
     PG3_CUDA(s, launch_pdl(pgk::rows_inv_kernel<M, true>, dim3(rgrid_inv), dim3(RSI::THREADS), RSI::SMEM, st, (const cplx *)in->d_W,
                            d_phi, (const cplx *)in->d_tw_row, (const double *)s->d_ones, N, n_items, ws, (long)N * N, CUtensorMap{}));
     in->launches++;
+    // rows_inv_kernel releases its dependents before it has finished writing: a polar solver on this stream that is
+    // fed Phi as its density must not fetch it early (same per-stream record as launch_rows_inv keeps)
+    note_early_release_output(s->device, st, d_phi, (size_t)N * N * N * sizeof(double));
     PG3_CUDA(s, cudaGetLastError());
     return PG_OK;
 }
@@ -1563,9 +1574,11 @@ pg_status pg3_create(pg3_solver **out, int n, double box, int device, void *cuda
     if (e == cudaSuccess) e = cudaMalloc((void **)&s->d_ones, n * sizeof(double));
     if (e == cudaSuccess) e = cudaMemcpy(s->d_ones, ones.data(), n * sizeof(double), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) {
-        set_err3(nullptr, "device allocation failed: %s", cudaGetErrorString(e));
+        const bool nomem = e == cudaErrorMemoryAllocation;
+        set_err3(nullptr, nomem ? "device allocation failed: %s" : "pg3_create: CUDA error while setting up the mesh: %s", cudaGetErrorString(e));
+        (void)cudaGetLastError();
         cart_free(s);
-        return PG_ERR_NOMEM;
+        return nomem ? PG_ERR_NOMEM : PG_ERR_CUDA;
     }
     rc = cart_build(s);
     if (rc != PG_OK) {
@@ -1831,7 +1844,7 @@ pg_status pg3n_add_exterior(pg3n_level *s, const double *parent_halo)
     if (!s->solved) { set_err3n(s, "pg3n_add_exterior before pg3n_solve"); return PG_ERR_STATE; }
     if (s->level == 0 && parent_halo) { set_err3n(s, "level 0 is isolated: parent_halo must be NULL"); return PG_ERR_INVALID_ARG; }
     if (s->level > 0 && !parent_halo) {        // one-sided: what the parent has put into this level's inbox
-        if (!s->inbox[PG3N_INBOX_HALO]) { set_err3n(s, "parent_halo is NULL and this level has no HALO inbox (pg3n_inbox_export)"); return PG_ERR_INVALID_ARG; }
+        if (!s->inbox[PG3N_INBOX_HALO]) { set_err3n(s, "parent_halo is NULL and this level has no HALO inbox (pg3n_inbox_export)"); return PG_ERR_STATE; }
         parent_halo = s->inbox[PG3N_INBOX_HALO];
     }
     if (s->level > 0 && !dev_ptr_ok(s, parent_halo, "parent_halo")) return PG_ERR_INVALID_ARG;

@@ -375,3 +375,69 @@ def test_fused_solves_on_four_lanes_equal_the_ordinary_path(n_r, n_phi):
             assert np.array_equal(a, b) and (a < 0).all()
     finally:
         s.close()
+
+
+@pytest.mark.parametrize("batch", [1, 3])
+def test_lanes_with_a_device_density_and_a_host_potential_stay_on_the_solvers_stream(batch):
+    """PG_OPT_LANES >= 2 + PG_OPT_DENSITY_STABLE, device Sigma, HOST Phi: the staged download waits for events on the
+    solver's stream, so these solves must not go to a lane (polargrav.h: host memspaces keep using the solver's stream).
+    Before the fix field 0 was solved on a lane stream and its download could run ahead of it (stale data)."""
+    n_r, n_phi = 256, 512
+    st = torch.cuda.Stream()
+    s = pg.Solver(n_r, n_phi, 1.0, 1000.0, 0.01, max_batch=batch, device=0, cuda_stream=st.cuda_stream)
+    pin = pg.PinnedArray((batch, n_r, n_phi))
+    try:
+        pg.pg_set_option(s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        K = 6
+        sig = [torch.from_numpy(np.stack([random_sigma(n_r, n_phi, 1300 + 10 * k + b) for b in range(batch)])).cuda() for k in range(K)]
+        torch.cuda.synchronize()
+
+        def run(lanes, where):
+            pg.pg_set_option(s.h, pg.PG_OPT_LANES, lanes)
+            res = []
+            for k in range(K):
+                pg.pg_set_density(s.h, sig[k], batch, pg.PG_MEM_DEVICE)
+                if where == pg.PG_MEM_HOST:
+                    out = np.full((batch, n_r, n_phi), np.nan)
+                    pg.pg_potential(s.h, out, batch, where)            # blocks until filled
+                    res.append(out)
+                else:
+                    pin.array[...] = np.nan
+                    pg.pg_potential(s.h, pin.ptr, batch, where)
+                    pg.pg_synchronize(s.h)
+                    res.append(pin.array.copy())
+            return res
+
+        one = run(1, pg.PG_MEM_HOST)
+        assert all((x < 0).all() for x in one)
+        for lanes in (2, 4):
+            for where in (pg.PG_MEM_HOST, pg.PG_MEM_HOST_PINNED):
+                for a, b in zip(one, run(lanes, where)):
+                    assert np.array_equal(a, b)
+    finally:
+        pin.free()
+        s.close()
+
+
+def test_profiling_survives_a_solve_with_non_symmetric_softening(solver):
+    """pg_profile(1) + PG_SOFT_FIELD / PG_SOFT_SOURCE: the variant path records no per-kernel events, so it must not take
+    a profiling slot; afterwards pg_kernel_times, pg_profile and pg_set_stream keep working and the counters hold only
+    the symmetric solves."""
+    sig = random_sigma(N_R, N_PHI, 77)
+    d_s = torch.from_numpy(sig).cuda()
+    d_p = torch.empty_like(d_s)
+    pg.pg_set_density(solver.h, d_s, 1, pg.PG_MEM_DEVICE)
+    pg.pg_profile(solver.h, True)
+    pg.pg_potential(solver.h, d_p, 1, pg.PG_MEM_DEVICE)
+    for soft in (pg.PG_SOFT_FIELD, pg.PG_SOFT_SOURCE):
+        pg.pg_set_softening(solver.h, soft)
+        pg.pg_potential(solver.h, d_p, 1, pg.PG_MEM_DEVICE)
+        ms, n = pg.pg_kernel_times(solver.h)
+        assert n == [1, 1, 1]
+    pg.pg_set_softening(solver.h, pg.PG_SOFT_SYMMETRIC)
+    pg.pg_potential(solver.h, d_p, 1, pg.PG_MEM_DEVICE)
+    ms, n = pg.pg_kernel_times(solver.h)
+    assert n == [2, 2, 2] and all(t > 0 for t in ms)
+    pg.pg_profile(solver.h, False)
+    pg.pg_set_stream(solver.h, torch.cuda.current_stream().cuda_stream)
+    pg.pg_synchronize(solver.h)

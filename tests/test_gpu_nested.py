@@ -86,7 +86,7 @@ def test_coupling_kernels_step_by_step_and_call_order_errors():
         pg.pg3n_pack_exterior(h0, halo)
         with pytest.raises(pg.PolargravError) as e:            # level 1 needs its parent's values
             pg.pg3n_add_exterior(h1, None)
-        assert e.value.status == pg.PG_ERR_INVALID_ARG
+        assert e.value.status == pg.PG_ERR_STATE             # no inbox yet: a state error, like restrict / absorb / pack
         pg.pg3n_add_exterior(h1, halo)
         out0 = np.empty((n, n, n)); out1 = np.empty((n, n, n))
         pg.pg3n_potential(h0, out0, pg.PG_MEM_HOST); pg.pg3n_potential(h1, out1, pg.PG_MEM_HOST)
