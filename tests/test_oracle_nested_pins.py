@@ -154,3 +154,93 @@ def test_against_the_direct_sum_over_the_composite_mass_distribution():
     assert rel.max() < 2e-2
     share = np.abs(ext).min() / np.abs(direct).max()
     assert share > 0.1                                    # the exterior term matters in this configuration
+
+
+# ------------------------------------------------------------------ depth >= 3: the recursion of M4, E_(l+1) = P[out_l + E_l]
+# ext[0] is zero, so the "+ E_l" inside the prolongation only acts from the third level on (the paper's hierarchy has
+# four, Fig. 8).  Both tests below turn red when nested_potential prolongs out_l alone.
+
+def _point_sources_potential(tgt_axes, src_pos, src_m):
+    """-sum m / |x - x'| at the tensor grid of the three target axes ([z][y][x]); sources as point masses"""
+    z, y, x = tgt_axes
+    out = np.zeros((len(z), len(y), len(x)))
+    for p, m in zip(src_pos, src_m):
+        out -= m / np.sqrt((z[:, None, None] - p[0]) ** 2 + (y[None, :, None] - p[1]) ** 2 + (x[None, None, :] - p[2]) ** 2)
+    return out
+
+
+def test_far_point_mass_on_level_0_reaches_level_2_through_two_prolongations():
+    """One massive cell on level 0 outside box_1, levels 1 and 2 empty: out_1 = 0, so everything level 2 sees comes
+    through E_1 inside P[out_1 + E_1].  Phi_2 = -M/d within the bound of two trilinear interpolations; without the
+    recursion term Phi_2 is identically zero."""
+    n, box = 32, 8.0
+    h0, h1 = box / n, box / 2 / n
+    coarse = np.zeros((n, n, n)); coarse[16, 15, 1] = 5.0           # [z][y][x]: 7 cells outside box_1 in x
+    empty = np.zeros((n, n, n))
+    phi, _ = no.nested_potential(n, box, [coarse, empty, empty])
+    x0, x1, x2 = centres(n, box, 0), centres(n, box, 1), centres(n, box, 2)
+    m = 5.0 * h0**3
+    src = np.array([x0[16], x0[15], x0[1]])
+    d2 = np.sqrt((x2[:, None, None] - src[0]) ** 2 + (x2[None, :, None] - src[1]) ** 2 + (x2[None, None, :] - src[2]) ** 2)
+    exact = -m / d2
+    assert np.abs(phi[2]).min() > 0.5 * np.abs(exact).min()          # not zero: the recursion term is there
+    rel = np.abs(phi[2] / exact - 1)
+    # first interpolation (level 0 -> 1), only its values on the level-1 cells that level 2 reads, [n/4 - 1, 3n/4]:
+    # |e1| <= (3/4) (h0/d)^2 |f| there (same bound as the depth-2 test); the second one is a convex combination of them
+    # (weights >= 0, sum 1), so it passes max |e1| on and adds (3/4) (h1/d)^2 |f| of its own.
+    q = n // 4
+    x1h = x1[q - 1:3 * q + 1]
+    d1 = np.sqrt((x1h[:, None, None] - src[0]) ** 2 + (x1h[None, :, None] - src[1]) ** 2 + (x1h[None, None, :] - src[2]) ** 2)
+    e1_abs = (0.75 * (h0 / d1) ** 2 * m / d1).max()
+    bound = e1_abs / np.abs(exact).min() + 0.75 * (h1 / d2.min()) ** 2
+    assert rel.max() < bound
+    assert bound < 0.02                                               # and the bound is tight enough to mean something
+    # level 1 itself, for completeness: one interpolation
+    d1f = np.sqrt((x1[:, None, None] - src[0]) ** 2 + (x1[None, :, None] - src[1]) ** 2 + (x1[None, None, :] - src[2]) ** 2)
+    assert np.abs(phi[1] / (-m / d1f) - 1).max() < 0.75 * (h0 / d1f.min()) ** 2
+
+
+def test_depth_three_against_the_direct_sum_over_the_composite_mass_distribution():
+    """Depth 3.  Mass on level 0 only in its outermost layer of cells, on level 1 only in ITS outermost layer, a blob on
+    level 2: every exterior source is many cells away from where its potential is interpolated, so the error of the
+    scheme against the plain sum over the leaf cells is bounded by the trilinear bound source by source,
+        |error of Phi_2| <= b0 |Phi_2 from level 0| + b1 |Phi_2 from level 1|     (all contributions have one sign),
+    b0 for two interpolations (h0 then h1), b1 for one (h1).  The level-0 share of Phi_2 is > 10 % and many times that
+    bar: prolonging out_1 without E_1 fails it."""
+    n, box = 32, 8.0
+    h = [box / 2**l / n for l in range(3)]
+    x = [centres(n, box, l) for l in range(3)]
+    rng = np.random.default_rng(31)
+    shell = np.zeros((n, n, n), bool)
+    shell[[0, -1], :, :] = True; shell[:, [0, -1], :] = True; shell[:, :, [0, -1]] = True
+    rho0 = np.where(shell, 3.0 + rng.random((n, n, n)), 0.0)
+    rho1 = np.where(shell, 1.0 + rng.random((n, n, n)), 0.0)
+    g2 = np.exp(-(x[2][:, None, None] ** 2 + x[2][None, :, None] ** 2 + x[2][None, None, :] ** 2) / (2 * 0.3**2))
+    rho2 = 2.0 * g2 + 0.05
+    phi, _ = no.nested_potential(n, box, [rho0, rho1, rho2])
+
+    def leaves(l, rho):
+        zz, yy, xx = np.meshgrid(x[l], x[l], x[l], indexing="ij")
+        return np.stack([zz[shell], yy[shell], xx[shell]], axis=1), rho[shell] * h[l] ** 3
+    p0, m0 = leaves(0, rho0)
+    p1, m1 = leaves(1, rho1)
+    axes2 = (x[2], x[2], x[2])
+    from0, from1 = _point_sources_potential(axes2, p0, m0), _point_sources_potential(axes2, p1, m1)
+    own2 = oracle.cart_potential(n, box / 4, rho2)
+    # the centre of level 1 is replaced by the means of level 2 (M2) and solved by level 2 itself; nothing else is inside
+    direct = own2 + from0 + from1
+    err = np.abs(phi[2] - direct)
+    # distances: level-0 shell at |coordinate| >= box/2 - h0 on some axis; it is interpolated first onto the level-1 cells
+    # level 2 reads (|coordinate| <= box/8 + 1.5 h1), then onto level 2 (|coordinate| <= box/8); the level-1 shell likewise
+    d01 = (box / 2 - h[0]) - (box / 8 + 1.5 * h[1])
+    d02 = (box / 2 - h[0]) - box / 8
+    d12 = (box / 4 - h[1]) - box / 8
+    # |f| at the level-1 cells read may exceed |f| at the level-2 target by at most the ratio of the distances
+    b0 = 0.75 * (h[0] / d01) ** 2 * (d02 + np.sqrt(3) * box / 4) / d01 + 0.75 * (h[1] / d02) ** 2
+    b1 = 0.75 * (h[1] / d12) ** 2
+    bar = b0 * np.abs(from0) + b1 * np.abs(from1)
+    assert (err < bar).all()
+    assert (bar / np.abs(direct)).max() < 0.02                           # a bar of under 2 % of Phi_2 everywhere
+    share0 = np.abs(from0) / np.abs(direct)
+    print(f"err/bar max {(err / bar).max():.3f}  level-0 share min {share0.min():.3f}  from0/bar min {(np.abs(from0) / bar).min():.1f}")
+    assert share0.min() > 0.10 and (np.abs(from0) / bar).min() > 10      # dropping E_1 inside P[...] is >= 10 bars off
