@@ -117,3 +117,18 @@ def random_sigma(n_r: int, n_phi: int, seed: int, signed: bool = False) -> np.nd
     rng = np.random.Generator(np.random.PCG64(seed))
     s = rng.random((n_r, n_phi))
     return s - 0.5 if signed else s
+
+
+def make_rho3(n: int, seed: int) -> np.ndarray:
+    """Synthetic 3-D mesh level [z][y][x] in the spirit of the paper's runs, whose contents are never described
+    (PAPER.md:271): a centrally condensed clump, six seeded Gaussian clumps, 1 % noise; non-negative.  The one generator
+    for bench.py --cart / --nested and tests/test_gpu_cartesian.py (inputs only, none of the method's arithmetic)."""
+    rng = np.random.Generator(np.random.PCG64(2409022940 + 1000 * n + seed))
+    z, y, x = np.meshgrid(*(np.arange(n) + 0.5,) * 3, indexing="ij")
+    c = n / 2.0
+    rho = 1.0 / (1.0 + ((x - c) ** 2 + (y - c) ** 2 + (z - c) ** 2) / (0.1 * n) ** 2)
+    for _ in range(6):
+        cx, cy, cz = rng.uniform(0.2 * n, 0.8 * n, 3)
+        w = rng.uniform(1.5, 4.0)
+        rho += rng.uniform(0.5, 3.0) * np.exp(-((x - cx) ** 2 + (y - cy) ** 2 + (z - cz) ** 2) / (2 * w * w))
+    return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))

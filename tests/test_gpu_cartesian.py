@@ -8,23 +8,9 @@ torch = pytest.importorskip("torch")
 
 import oracle
 from paper_2409_02294_b200 import binding as pg
+from paper_2409_02294_b200.workloads import make_rho3 as make_rho
 
 pytestmark = pytest.mark.gpu
-
-
-def make_rho(n, seed):
-    """Synthetic mesh level in the spirit of the paper's runs (contents never described): a centrally
-    condensed clump plus a few seeded Gaussian clumps plus 1 % noise; non-negative."""
-    rng = np.random.Generator(np.random.PCG64(2409022940 + 1000 * n + seed))
-    z, y, x = np.meshgrid(*(np.arange(n) + 0.5,) * 3, indexing="ij")
-    c = n / 2.0
-    r2 = (x - c) ** 2 + (y - c) ** 2 + (z - c) ** 2
-    rho = 1.0 / (1.0 + r2 / (0.1 * n) ** 2)
-    for _ in range(6):
-        cx, cy, cz = rng.uniform(0.2 * n, 0.8 * n, 3)
-        w = rng.uniform(1.5, 4.0)
-        rho += rng.uniform(0.5, 3.0) * np.exp(-((x - cx) ** 2 + (y - cy) ** 2 + (z - cz) ** 2) / (2 * w * w))
-    return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))
 
 
 class Dev3:
@@ -59,8 +45,20 @@ def test_cartesian_32_every_cell():
         d.close()
 
 
-@pytest.mark.parametrize("n,n_targets", [(64, 2048), (128, 512), (256, 64)])
+def whole_lines(n):
+    """Flat indices of the six whole lines along x, y and z through the corner cell (0, 0, 0) and through the centre
+    cell: every x of a row, every y of a column, every z of a pillar -- all the tiles the transposing y pass
+    (ycols_fwd / ycols_inv, runs of YM columns) and the row kernels cut a line into, first and last included."""
+    a, c = np.arange(n), n // 2
+    flat = lambda z, y, x: (z * n + y) * n + x
+    return np.concatenate([flat(0, 0, a), flat(0, a, 0), flat(a, 0, 0), flat(c, c, a), flat(c, a, c), flat(a, c, c)])
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("n,n_targets", [(64, 2048), (128, 20000), (256, 2000)])
 def test_cartesian_sampled_targets_at_the_papers_sizes(n, n_targets):
+    """64^3 and 128^3 are the paper's sizes.  The oracle costs n^3 pair terms per target: 20 000 targets at
+    128^3 and 2 000 at 256^3 are ~4e10 terms each (tens of seconds on the host cores)."""
     box = 10.0
     d = Dev3(n, box)
     try:
@@ -69,24 +67,30 @@ def test_cartesian_sampled_targets_at_the_papers_sizes(n, n_targets):
         assert np.isfinite(got).all() and (got < 0).all()
         rng = np.random.default_rng(n)
         corners = [0, n - 1, n * n - 1, n**3 - 1, (n // 2) * (n * n + n + 1)]
-        tg = np.unique(np.concatenate([corners, rng.integers(0, n**3, n_targets)])).astype(np.int64)
+        lines = whole_lines(n)
+        tg = np.unique(np.concatenate([corners, lines, rng.integers(0, n**3, n_targets - len(lines))])).astype(np.int64)
+        assert len(tg) >= 0.99 * n_targets
         ref = oracle.cart_potential_targets(n, box, rho, tg)
         check(got.reshape(-1)[tg], ref, f"{n}^3 on {len(tg)} sampled cells")
+        ln = np.isin(tg, lines)
+        check(got.reshape(-1)[tg[ln]], ref[ln], f"{n}^3 on the six whole lines")
     finally:
         d.close()
 
 
-def test_cartesian_single_cell_no_wraparound_and_self_term():
-    """A unit cell in a corner: Phi = -h^3 / distance everywhere (no periodic image leaks in through the padding),
-    -h^2 S in the cell itself."""
-    n, box = 64, 64.0
+@pytest.mark.parametrize("n", [64, 128, 256])
+def test_cartesian_single_cell_no_wraparound_and_self_term(n):
+    """A unit cell in a corner, on a face, in the centre: Phi = -h^3 / distance on EVERY cell (no periodic image leaks in
+    through the padding), -h^2 S in the cell itself.  The closed form costs numpy nothing, so the paper's 128^3
+     and 256^3 are checked whole: an index slip in a tile of the transposing y pass cannot hide."""
+    box = float(n)
     d = Dev3(n, box)
     try:
-        for pos in ((0, 0, 0), (n - 1, n - 1, n - 1), (n - 1, 0, n // 2)):
+        a = np.arange(n, dtype=np.float64)
+        for pos in ((0, 0, 0), (n - 1, n - 1, n - 1), (n - 1, 0, n // 2), (n // 2, n // 2, n // 2), (3, n // 2 + 1, n - 2)):
             rho = np.zeros((n, n, n)); rho[pos] = 1.0
             got = d.solve(rho)
-            z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
-            dist = np.sqrt((z - pos[0]) ** 2.0 + (y - pos[1]) ** 2.0 + (x - pos[2]) ** 2.0)
+            dist = np.sqrt(((a - pos[0]) ** 2)[:, None, None] + ((a - pos[1]) ** 2)[None, :, None] + ((a - pos[2]) ** 2)[None, None, :])
             with np.errstate(divide="ignore"):
                 expect = -1.0 / dist
             expect[pos] = -(3 * np.log(2 + np.sqrt(3)) - np.pi / 2)

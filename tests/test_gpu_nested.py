@@ -35,7 +35,7 @@ def check(got, ref, what):
     assert l2 <= 1e-10 and mx <= 1e-9, f"{what}: rel-L2 {l2:.3e}, max rel {mx:.3e}"
 
 
-@pytest.mark.parametrize("n,depth", [(32, 1), (32, 2), (32, 3), (64, 2)])
+@pytest.mark.parametrize("n,depth", [(32, 1), (32, 2), (32, 3), (32, 4), (64, 2)])      # depth 4: the paper's hierarchy, Fig. 8
 def test_nested_levels_on_one_gpu_vs_oracle(n, depth):
     box0 = 8.0
     rhos = [level_rho(n, l, depth) for l in range(depth)]
@@ -101,6 +101,54 @@ def test_coupling_kernels_step_by_step_and_call_order_errors():
         assert np.abs(ext1 - no.prolong(got_halo, n)).max() <= 1e-11 * np.abs(out1).max()
     finally:
         pg.pg3n_destroy(h0); pg.pg3n_destroy(h1)
+
+
+@pytest.mark.parametrize("n", [64, 128])
+def test_coupling_kernels_at_the_papers_mesh_sizes(n):
+    """The five coupling kernels (restrict, absorb, mask, pack, prolong) at 64^3 and 128^3 against the numpy
+    oracle steps.  The oracle's per-level solve costs n^6 and is out of reach here, so the single-level solves the
+    coupling sits between are taken from pg3_potential -- the path test_gpu_cartesian.py holds to the oracle -- and only
+    the coupling arithmetic is under test: copies and the 8-child mean must be exact, the trilinear sum within rounding."""
+    box0 = 4.0
+    rng = np.random.default_rng(100 + n)
+    coarse, fine = rng.random((n, n, n)), rng.random((n, n, n))
+    st = torch.cuda.current_stream().cuda_stream
+    h0 = pg.pg3n_create(n, box0, 0, 2, 0, st)
+    h1 = pg.pg3n_create(n, box0, 1, 2, 0, st)
+    m0, m1 = pg.pg3_create(n, box0, 0, st), pg.pg3_create(n, box0 / 2, 0, st)
+
+    def single(mesh, rho):
+        d_r = torch.from_numpy(np.ascontiguousarray(rho)).cuda(); d_p = torch.empty_like(d_r)
+        pg.pg3_set_density(mesh, d_r, pg.PG_MEM_DEVICE)
+        pg.pg3_potential(mesh, d_p, pg.PG_MEM_DEVICE)
+        pg.pg3_synchronize(mesh)
+        return d_p.cpu().numpy()
+
+    try:
+        n_mean, n_halo = nested.message_counts(n)
+        mean = torch.zeros(n_mean, dtype=torch.float64, device="cuda")
+        halo = torch.zeros(n_halo, dtype=torch.float64, device="cuda")
+        pg.pg3n_set_density(h0, torch.from_numpy(coarse).cuda(), pg.PG_MEM_DEVICE)
+        pg.pg3n_set_density(h1, torch.from_numpy(fine).cuda(), pg.PG_MEM_DEVICE)
+        pg.pg3n_restrict(h1, mean)
+        pg.pg3n_synchronize(h1)
+        got_mean = mean.cpu().numpy().reshape((n // 2,) * 3)
+        assert np.array_equal(got_mean, no.restrict(fine))                                        # restrict (M2)
+        pg.pg3n_absorb(h0, mean)
+        pg.pg3n_solve(h0); pg.pg3n_solve(h1)
+        pg.pg3n_add_exterior(h0, None)
+        pg.pg3n_pack_exterior(h0, halo)
+        pg.pg3n_add_exterior(h1, halo)
+        out0, out1 = np.empty((n, n, n)), np.empty((n, n, n))
+        pg.pg3n_potential(h0, out0, pg.PG_MEM_HOST); pg.pg3n_potential(h1, out1, pg.PG_MEM_HOST)
+        rho0 = no.absorb(coarse, got_mean)
+        assert np.array_equal(out0, single(m0, rho0))                                             # absorb (M2); E_0 = 0 (M6)
+        got_halo = halo.cpu().numpy().reshape((n // 2 + 2,) * 3)
+        assert np.array_equal(got_halo, no.pack_halo(single(m0, no.mask_centre(rho0))))           # mask (M3) + pack (M5)
+        want1 = single(m1, fine) + no.prolong(got_halo, n)                                        # prolong (M5) + M6
+        assert np.abs(out1 / want1 - 1.0).max() <= 1e-15 * 8
+    finally:
+        pg.pg3n_destroy(h0); pg.pg3n_destroy(h1); pg.pg3_destroy(m0); pg.pg3_destroy(m1)
 
 
 # ------------------------------------------------------------------ one level per process, one-sided exchange
