@@ -31,7 +31,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2409_02294_b200.workloads import CONFIGS, make_sigma  # noqa: E402
+from paper_2409_02294_b200.workloads import CONFIGS, make_rho3, make_sigma  # noqa: E402
 from paper_2409_02294_b200 import replicas  # noqa: E402
 
 METRIC = "potential solves/sec (fp64 FFT-convolution, log-polar thin disk)"
@@ -259,7 +259,8 @@ def workload_name(cfg: int) -> str:
 
 
 # ------------------------------------------------------------------ the CUDA path
-def run_ours(args):
+def measure_ours(args):
+    """The main line (2-D path, BASELINE.json's metric) as a dict, and the exit code of its parity gate; prints nothing."""
     import torch
     from paper_2409_02294_b200 import binding as pg, build as pg_build
 
@@ -373,6 +374,24 @@ def run_ours(args):
     value = world * c.batch * 1e3 / ms_per_step
     n_launch = int(round((n1 - n0) / REPEATS)) * world
 
+    # ---- the same K-step region with ONE solve in flight (PG_OPT_LANES = 1): what a time series gets whose step k + 1
+    # depends on step k (a disk code that evolves Sigma with Phi), SURVEY 8(d)'s "one stream" protocol
+    ms_one_lane = ms_per_step
+    if lanes >= 2:
+        pg.pg_set_option(h, pg.PG_OPT_LANES, 1)
+        one = []
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier(); torch.cuda.synchronize()
+            e0.record(st)
+            for k in range(args.steps):
+                step(k)
+            e1.record(st)
+            torch.cuda.synchronize(); barrier()
+            one.append(max_over_ranks(e0.elapsed_time(e1)))
+        ms_one_lane = float(np.median(one)) / args.steps
+        pg.pg_set_option(h, pg.PG_OPT_LANES, lanes)
+
     # ---- per-kernel durations (events around every kernel, separate pass) -> roofline of the dominant kernel
     pg.pg_profile(h, True)
     for k in range(args.steps):
@@ -385,6 +404,8 @@ def run_ours(args):
     ncu, ncu_why = ncu_record(cfg) if not args.batch else (None, "--batch overrides the config the ncu record was captured at")
     kbytes = [pg.pg_kernel_algorithmic_bytes(h, i, c.batch) for i in range(pg.PG_NUM_KERNELS)]
     achieved = kbytes[dom] / (per_launch_ms[dom] * 1e-3) / 1e9
+    # the bytes the kernel has to move as built: the column kernel reads Khat as its symmetric half (8 N_r M_h bytes less)
+    needed = kbytes[dom] - (8.0 * c.n_r * (c.n_phi // 2 + 1) if dom == 1 else 0.0)
     path_bytes = pg.pg_algorithmic_bytes(h, c.batch)
     path_gbs = path_bytes / (ms_per_step * 1e-3) / 1e9
 
@@ -438,7 +459,8 @@ def run_ours(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_step_one_lane": ms_one_lane,
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg) + (f" -- OVERRIDDEN: batch {c.batch} (--batch; not a BASELINE.json workload)" if args.batch else ""),
                    "n_r": c.n_r, "n_phi": c.n_phi, "batch": c.batch,
@@ -458,7 +480,8 @@ def run_ours(args):
         "host": host_placement(local_rank),
         "roofline": {
             "bound": "hbm", "kernel": pg.KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "traffic": (ncu or {}).get("dram_bytes_per_launch", [None] * 3)[dom],
+            "frac": achieved / peak, "frac_needed_bytes": needed / (per_launch_ms[dom] * 1e-3) / 1e9 / peak,
+            "needed_bytes_per_launch": needed, "traffic": (ncu or {}).get("dram_bytes_per_launch", [None] * 3)[dom],
             "traffic_source": (f"profiles/ncu_head.json, ncu --set full at commit {ncu['commit']}" if ncu else ncu_why),
             "peak_source": peak_src,
             "algorithmic_bytes_per_launch": kbytes[dom], "ms_per_launch": per_launch_ms[dom],
@@ -471,7 +494,13 @@ def run_ours(args):
             "path": {"alg_bytes_per_step": path_bytes, "gbs": path_gbs, "frac_of_peak": path_gbs / peak,
                      "frac_of_8TBs_nominal": path_gbs / 8000.0},
             "fp64": fp64_block((ncu or {}).get("fp64_thread_instructions_per_launch", [None] * 3)[dom], per_launch_ms[dom], clocks),
-            "l2_flushed_ms_per_step": ms_flushed, "l2_flushed_frac_of_peak": path_bytes / (ms_flushed * 1e-3) / 1e9 / peak,
+            "one_lane": {"ms_per_step": ms_one_lane, "gbs": path_bytes / (ms_one_lane * 1e-3) / 1e9,
+                         "frac_of_peak": path_bytes / (ms_one_lane * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBs_nominal": path_bytes / (ms_one_lane * 1e-3) / 1e9 / 8000.0},
+            "l2_flushed_one_lane_serialised": {
+                "ms_per_step": ms_flushed, "frac_of_peak": path_bytes / (ms_flushed * 1e-3) / 1e9 / peak,
+                "note": "one solve at a time, each timed on its own behind a > L2 memset: NOT comparable with ms_per_step "
+                        "(no overlap between solves, cold L2 for Khat and the tables); compare with one_lane"},
         },
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": field_bytes * c.batch,
                 "d2h_bytes_per_step": field_bytes * c.batch,
@@ -492,12 +521,56 @@ def run_ours(args):
         import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()
+    return line, (0 if parity["ok"] else 3)
+
+
+def compact(line):
+    """The figures of a secondary line that the main line carries in its `others` block."""
+    rf = line.get("roofline", {})
+    path = rf.get("path", {})
+    par = line.get("parity", {})
+    return {"workload": line["config"]["workload"], "steps": line["steps"], "ms_per_step": line["ms_per_step"],
+            "value": line["value"], "unit": line["unit"], "cells_per_s": line.get("cells_per_s"),
+            "gpu_launches": line.get("gpu_launches"),
+            "parity": {k: par.get(k) for k in ("rel_l2", "max_rel", "ok", "what")},
+            "path_gbs": path.get("gbs", rf.get("achieved")),
+            "path_frac_of_peak": path.get("frac_of_peak", rf.get("frac")),
+            "path_frac_of_8TBs_nominal": path.get("frac_of_8TBs_nominal", (rf.get("achieved") or 0.0) / 8000.0),
+            "clocks_sm_mhz": (line.get("clocks") or {}).get("sm_mhz")}
+
+
+def others_block(args):
+    """Driver-witnessed figures for the workloads the default line is NOT quoted on: config 4 (8 x 1024^2), one 128^3
+    Cartesian mesh level (NEXT-2) and four nested 64^3 levels (NEXT-3), 20 steps each with their own parity gates, same
+    protocol as their own modes (--config 4, --cart 128, --nested 4 --cart 64), no oracle timing."""
+    import copy
+    out, rc = {}, 0
+    for key, kw, fn in (("config4", dict(config=4), measure_ours), ("cart128", dict(cart=128), measure_cart),
+                        ("nested4x64", dict(nested=4, cart=64), measure_nested)):
+        a = copy.copy(args)
+        a.steps, a.warmup, a.no_cpu_baseline, a.lanes, a.batch = 20, 3, True, 0, 0
+        for k, v in kw.items():
+            setattr(a, k, v)
+        try:
+            line, r = fn(a)
+            out[key] = compact(line)
+            rc = rc or r
+        except Exception as e:                      # a secondary figure must not take the headline down with it
+            out[key] = {"error": f"{type(e).__name__}: {e}"}
+    return out, rc
+
+
+def run_ours(args):
+    line, rc = measure_ours(args)
+    rank, _, world = dist_env()
+    if rank == 0 and world == 1 and args.config == 5 and not args.batch and not args.no_others:
+        line["others"], rc_o = others_block(args)
+        rc = rc or rc_o
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if not parity["ok"]:
-        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {parity}; the timing above does not count\n")
-        return 3
-    return 0
+    if rc:
+        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {line['parity']} / others {json.dumps({k: v.get('parity', v) for k, v in line.get('others', {}).items()})}; the timing above does not count\n")
+    return rc
 
 
 def batched_small(cfg, st, args):
@@ -688,22 +761,7 @@ def run_staging(args):
     return 0
 
 
-def make_rho3(n: int, seed: int):
-    """Synthetic mesh level in the spirit of the paper's runs, whose contents are never described:
-    a centrally condensed clump, six seeded Gaussian clumps, 1 % noise; non-negative.  (Same recipe as
-    tests/test_gpu_cartesian.py.)"""
-    rng = np.random.Generator(np.random.PCG64(2409022940 + 1000 * n + seed))
-    z, y, x = np.meshgrid(*(np.arange(n) + 0.5,) * 3, indexing="ij")
-    c = n / 2.0
-    rho = 1.0 / (1.0 + ((x - c) ** 2 + (y - c) ** 2 + (z - c) ** 2) / (0.1 * n) ** 2)
-    for _ in range(6):
-        cx, cy, cz = rng.uniform(0.2 * n, 0.8 * n, 3)
-        w = rng.uniform(1.5, 4.0)
-        rho += rng.uniform(0.5, 3.0) * np.exp(-((x - cx) ** 2 + (y - cy) ** 2 + (z - cz) ** 2) / (2 * w * w))
-    return rho * (1.0 + 0.01 * rng.standard_normal(rho.shape))
-
-
-def run_nested(args):
+def measure_nested(args):
     """--nested D [--cart N]: the paper's distributed scheme (row NEXT-3): D nested mesh levels of N^3 cells
     (Fig. 8 :306; readings M1-M6).  One process: all levels on one GPU, one CUDA stream each.
     Under torchrun with WORLD_SIZE = D: one level per rank / GPU, the two level-boundary messages by NCCL send / recv.
@@ -816,15 +874,19 @@ def run_nested(args):
     }
     if world > 1:
         dist.barrier(); dist.destroy_process_group()
-    if rank == 0:
+    return line, (0 if parity["ok"] else 3)
+
+
+def run_nested(args):
+    line, rc = measure_nested(args)
+    if replicas.dist_env()[0] == 0:
         print(json.dumps(line), flush=True)
-    if not parity["ok"]:
-        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {parity}\n")
-        return 3
-    return 0
+    if rc:
+        sys.stderr.write(f"bench.py: PARITY GATE FAILED: {line['parity']}\n")
+    return rc
 
 
-def run_cart(args):
+def measure_cart(args):
     """--cart N: the paper's own per-GPU workload (row NEXT-2): potential of ONE 3-D Cartesian mesh level of N^3 cells
     (N = 64 or 128) by the zero-padded FFT convolution, device resident.  Same protocol as the main
     line: median of REPEATS repeats of the K-step region, buffer rotation beyond L2, parity gate against the 3-D oracle
@@ -926,33 +988,14 @@ def run_cart(args):
     }
     pin_in.free(); pin_out.free()
     pg.pg3_destroy(h)
+    return line, (0 if ok else 3)
+
+
+def run_cart(args):
+    line, rc = measure_cart(args)
     print(json.dumps(line), flush=True)
-    if not ok:
+    if rc:
         sys.stderr.write(f"bench.py: PARITY GATE FAILED: {line['parity']}\n")
-        return 3
-    return 0
-
-
-def run_pipes(args):
-    """--pipes: builds and runs the microbenchmarks of csrc/microbench/ -- pipes.cu (FP64 issue rate by operand pattern,
-    FP64 || shared-memory overlap, cost of scattered 16-byte accesses) and runs.cu (what the memory system delivers for
-    transposed accesses by run length and path, STG / LDG / TMA tiles; a 16 x 16 complex transpose by shuffles against
-    shared memory) -- the measurements behind the pipe model and the design choices of DESIGN.md section 7."""
-    out, status, rc = {}, [], 0
-    for name in ("pipes.cu", "runs.cu"):
-        src = os.path.join(ROOT, "paper_2409_02294_b200", "csrc", "microbench", name)
-        exe = os.path.join(tempfile.gettempdir(), f"pg_{name[:-3]}_{os.getpid()}")
-        subprocess.run([os.environ.get("NVCC", "nvcc"), "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, src], check=True)
-        res = subprocess.run([exe], capture_output=True, text=True)
-        os.unlink(exe)
-        for line in res.stdout.splitlines():
-            t = line.split()
-            if len(t) == 3 and t[0] != "status":
-                out[t[0]] = {"value": float(t[1]), "unit": t[2]}
-        status.append(f"{name}: " + (res.stdout.strip().splitlines()[-1] if res.stdout.strip() else res.stderr[-200:]))
-        rc = rc or res.returncode
-    print(json.dumps({"metric": "microbenchmarks (csrc/microbench/pipes.cu, runs.cu)", "n_gpus": 1, "results": out,
-                      "status": status}), flush=True)
     return rc
 
 
@@ -964,6 +1007,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="default line only: skip the `others` block (config 4, --cart 128, --nested 4 --cart 64 at 20 steps)")
     ap.add_argument("--lanes", type=int, default=0, choices=[0, 1, 2, 3, 4], help="solves in flight (0 = 2 for grids of 2^20 cells and more)")
     ap.add_argument("--nested", type=int, default=0, help="D nested 3-D mesh levels of --cart N cells per edge (row NEXT-3; default N = 64); under torchrun with WORLD_SIZE = D one level per GPU")
     ap.add_argument("--batch", type=int, default=0, help="override the config's batch (fields per call); not a BASELINE.json workload")
@@ -973,15 +1017,12 @@ def main():
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
                     help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")
-    ap.add_argument("--pipes", action="store_true", help="run the pipe microbenchmarks (csrc/microbench/pipes.cu)")
     ap.add_argument("--staging", action="store_true", help="time row a6 alone: pinned vs pageable staging of a 128^3 array (PAPER.md:119)")
     args = ap.parse_args()
     if args.direct:
         return run_direct(args)
     if args.staging:
         return run_staging(args)
-    if args.pipes:
-        return run_pipes(args)
     if args.nested:
         return run_nested(args)
     if args.cart:

@@ -745,15 +745,9 @@ pg_status solve_fields(pg_solver *s, const double *d_sigma, double *d_phi, cplx 
             return PG_OK;
         }
         const int early = overlaps_early_release_output(s->device, lst, d_sigma, (size_t)batch * s->field * sizeof(double)) ? 0 : 2;
-#ifdef PG_KERNEL_MASK          // tuning runs: a subset of the three kernels (results are then meaningless)
-        if ((PG_KERNEL_MASK & 1) && (st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early)) != PG_OK) return st;
-        if ((PG_KERNEL_MASK & 2) && (st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
-        if ((PG_KERNEL_MASK & 4) && (st = rows_inv(s, W, d_phi, batch, ws, fs, lst)) != PG_OK) return st;
-#else
         if ((st = rows_fwd(s, d_sigma, W, s->d_rs_in, s->n_r, batch, fs, ws, lst, early)) != PG_OK) return st;
         if ((st = cols(s, W, batch, ws, lst)) != PG_OK) return st;
         if ((st = rows_inv(s, W, d_phi, batch, ws, fs, lst)) != PG_OK) return st;
-#endif
         s->lane_used[L] = true;            // joined by pg_flush / pg_synchronize
         return PG_OK;
     }
