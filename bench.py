@@ -607,8 +607,28 @@ def batched_small(cfg, st, args):
                 ms.append(e0.elapsed_time(e1) / steps)
         launches = (pg.pg_launch_count(s.h) - n0) / ((REPEATS + 1) * steps)
         med = float(np.median(ms))
+        # un-batched, but one host call for the whole series: pg_potential_series over the B fields of a buffer, one
+        # solve (one fused launch) per field, four lanes
+        pg.pg_set_option(s.h, pg.PG_OPT_LANES, 4)
+        field = c.n_r * c.n_phi
+        ser = []
+        for rep in range(REPEATS + 1):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(st)
+            for k in range(steps):
+                pg.pg_potential_series(s.h, d_sig[k % R], d_phi[k % R], B, field)
+            pg.pg_flush(s.h)
+            e1.record(st)
+            torch.cuda.synchronize()
+            if rep:
+                ser.append(e0.elapsed_time(e1) / (steps * B))
+        ser_med = float(np.median(ser))
         return {"batch": B, "ms_per_batch": med, "solves_per_s": B * 1e3 / med, "launches_per_batch": launches,
-                "what": f"{B} independent fields per pg_set_density / pg_potential pair (resident), median of {REPEATS} repeats of {steps} batches"}
+                "what": f"{B} independent fields per pg_set_density / pg_potential pair (resident), median of {REPEATS} repeats of {steps} batches",
+                "series": {"ms_per_solve": ser_med, "solves_per_s": 1e3 / ser_med,
+                           "what": f"pg_potential_series: {B} single-field solves per host call, one launch set each, PG_OPT_LANES = 4, "
+                                   f"median of {REPEATS} repeats of {steps} calls"}}
     finally:
         s.close()
 

@@ -142,6 +142,20 @@ typedef enum { PG_SOFT_SYMMETRIC = 0, PG_SOFT_FIELD = 1, PG_SOFT_SOURCE = 2 } pg
 pg_status pg_set_softening(pg_solver *s, pg_softening mode);
 pg_status pg_acceleration(pg_solver *s, double *a_r, double *a_phi, int batch, pg_memspace where);
 
+/*
+ * pg_potential_series -- `count` single-field solves enqueued by ONE host call (time series
+ * and ensembles on small grids are bound by the host's per-call cost, not by the GPU):
+ *     Phi_k = potential of Sigma_k,   Sigma_k = sigma + k * stride,  Phi_k = phi + k * stride,   k = 0 .. count-1,
+ * exactly as `count` pairs  pg_set_density(s, Sigma_k, 1, PG_MEM_DEVICE); pg_potential(s, Phi_k, 1, PG_MEM_DEVICE)
+ * would, in that order, with the same kernels (bit-identical results) and the same ordering rules: on the solver's
+ * stream, or -- with PG_OPT_LANES >= 2 and PG_OPT_DENSITY_STABLE -- dealt out to the lanes and complete after
+ * pg_flush / pg_synchronize.  The fields are independent of each other (Sigma_k is not read from Phi_(k-1)).
+ *   sigma, phi  device memory of the solver's device, 16-byte aligned; the two ranges of count * stride doubles may
+ *               not overlap.   stride  in doubles, even, >= n_r * n_phi.   count >= 1 (not limited by max_batch).
+ * Returns after enqueue; afterwards the density last set is Sigma_(count-1) with batch 1.
+ */
+pg_status pg_potential_series(pg_solver *s, const double *sigma, double *phi, int count, size_t stride);
+
 /* pg_destroy -- frees everything the solver owns. pg_destroy(NULL) is a no-op returning PG_OK. */
 pg_status pg_destroy(pg_solver *s);
 

@@ -31,7 +31,7 @@ EXPORTS = (
     "pg_potential_direct_rings", "pg_destroy", "pg_grid", "pg_set_stream", "pg_set_option", "pg_synchronize",
     "pg_host_alloc", "pg_host_free", "pg_profile", "pg_kernel_times", "pg_launch_count",
     "pg_algorithmic_bytes", "pg_kernel_algorithmic_bytes", "pg_status_string", "pg_last_error",
-    "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush", "pg_potential_direct_static",
+    "pg_version", "pg_set_softening", "pg_acceleration", "pg_flush", "pg_potential_direct_static", "pg_potential_series",
     "pg3_create", "pg3_set_density", "pg3_potential", "pg3_synchronize", "pg3_destroy", "pg3_launch_count",
     "pg3_algorithmic_bytes", "pg3_last_error",
     "pg3n_create", "pg3n_set_density", "pg3n_restrict", "pg3n_absorb", "pg3n_solve", "pg3n_add_exterior",
@@ -63,6 +63,7 @@ def lib():
         L.pg_set_density.argtypes = [vp, vp, i, i]
         L.pg_potential.argtypes = [vp, vp, i, i]
         L.pg_potential_direct.argtypes = [vp, vp, i, i]
+        L.pg_potential_series.argtypes = [vp, vp, vp, i, ctypes.c_size_t]
         L.pg_potential_direct_rings.argtypes = [vp, vp, i, i, i]
         L.pg_set_softening.argtypes = [vp, i]
         L.pg_acceleration.argtypes = [vp, vp, vp, i, i]
@@ -164,6 +165,10 @@ def pg_set_density(h, sigma, batch, where):
 
 def pg_potential(h, phi, batch, where):
     _check(lib().pg_potential(h, _ptr(phi), batch, where), h)
+
+
+def pg_potential_series(h, sigma, phi, count, stride):
+    _check(lib().pg_potential_series(h, _ptr(sigma), _ptr(phi), count, stride), h)
 
 
 def pg_potential_direct(h, phi, batch, where):

@@ -1155,6 +1155,34 @@ pg_status pg_potential(pg_solver *s, double *phi, int batch, pg_memspace where)
     return potential_common(s, phi, batch, where, false, 0, -1);
 }
 
+pg_status pg_potential_series(pg_solver *s, const double *sigma, double *phi, int count, size_t stride)
+{
+    if (!s) return PG_ERR_INVALID_ARG;
+    if (!sigma || !phi || count < 1) { set_err(s, "pg_potential_series: sigma or phi is NULL, or count %d < 1", count); return PG_ERR_INVALID_ARG; }
+    if (stride < s->field || (stride & 1u)) {
+        set_err(s, "pg_potential_series: stride %zu must be even and >= n_r * n_phi = %zu doubles", stride, s->field);
+        return PG_ERR_INVALID_ARG;
+    }
+    if ((((uintptr_t)sigma | (uintptr_t)phi) & 15u) != 0) {
+        set_err(s, "pg_potential_series: sigma and phi must be 16-byte aligned device pointers");
+        return PG_ERR_INVALID_ARG;
+    }
+    const size_t span = ((size_t)(count - 1) * stride + s->field) * sizeof(double);
+    if (ranges_overlap(sigma, span, phi, span)) {
+        set_err(s, "pg_potential_series: the phi range overlaps the sigma range");
+        return PG_ERR_INVALID_ARG;
+    }
+    DeviceGuard guard(s->device);
+    s->sigma_from_host = false;
+    s->cur_batch = 1;
+    for (int k = 0; k < count; ++k) {
+        s->d_sigma = sigma + (size_t)k * stride;
+        pg_status st = solve_fields(s, s->d_sigma, phi + (size_t)k * stride, s->d_W, 1, true);
+        if (st != PG_OK) return st;
+    }
+    return PG_OK;
+}
+
 pg_status pg_potential_direct(pg_solver *s, double *phi, int batch, pg_memspace where)
 {
     return potential_common(s, phi, batch, where, true, 0, -1);

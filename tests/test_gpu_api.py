@@ -441,3 +441,50 @@ def test_profiling_survives_a_solve_with_non_symmetric_softening(solver):
     pg.pg_profile(solver.h, False)
     pg.pg_set_stream(solver.h, torch.cuda.current_stream().cuda_stream)
     pg.pg_synchronize(solver.h)
+
+
+@pytest.mark.parametrize("n_r,n_phi,lanes", [(64, 64, 1), (256, 128, 4), (512, 512, 2), (1024, 1024, 2)])
+def test_series_call_equals_the_same_solves_one_by_one(n_r, n_phi, lanes):
+    """pg_potential_series: `count` solves enqueued by one host call are the solves of `count` pg_set_density /
+    pg_potential pairs bit for bit -- fused small grids and the three-kernel path, with and without lanes, with a
+    stride larger than a field (the gap must stay untouched)."""
+    st = torch.cuda.Stream()
+    s = pg.Solver(n_r, n_phi, 1.0, 400.0, 0.02, device=0, cuda_stream=st.cuda_stream)
+    try:
+        count, field = 9, n_r * n_phi
+        stride = field + 6
+        sig = np.zeros((count, stride)); 
+        for k in range(count):
+            sig[k, :field] = random_sigma(n_r, n_phi, 2100 + k).ravel()
+        d_s = torch.from_numpy(sig).cuda()
+        one = torch.full_like(d_s, 7.0)
+        many = torch.full_like(d_s, 7.0)
+        torch.cuda.synchronize()
+        pg.pg_set_option(s.h, pg.PG_OPT_DENSITY_STABLE, 1)
+        for k in range(count):
+            pg.pg_set_density(s.h, d_s[k].data_ptr(), 1, pg.PG_MEM_DEVICE)
+            pg.pg_potential(s.h, one[k].data_ptr(), 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(s.h)
+        pg.pg_set_option(s.h, pg.PG_OPT_LANES, lanes)
+        for rep in range(2):
+            pg.pg_potential_series(s.h, d_s, many, count, stride)
+        pg.pg_flush(s.h)
+        st.synchronize()
+        a, b = one.cpu().numpy(), many.cpu().numpy()
+        assert np.array_equal(a, b)
+        assert (b[:, :field] < 0).all() and (b[:, field:] == 7.0).all()
+        # afterwards the density set is the last field
+        last = torch.empty(n_r, n_phi, dtype=torch.float64, device="cuda")
+        pg.pg_potential(s.h, last, 1, pg.PG_MEM_DEVICE)
+        pg.pg_synchronize(s.h)
+        assert np.array_equal(last.cpu().numpy().ravel(), b[count - 1, :field])
+        for bad in (lambda: pg.pg_potential_series(s.h, d_s, many, 0, stride),
+                    lambda: pg.pg_potential_series(s.h, d_s, many, count, field - 2),
+                    lambda: pg.pg_potential_series(s.h, d_s, many, count, field + 1),
+                    lambda: pg.pg_potential_series(s.h, d_s, d_s.data_ptr() + 16, 2, stride),
+                    lambda: pg.pg_potential_series(s.h, d_s.data_ptr() + 8, many, 2, stride)):
+            with pytest.raises(pg.PolargravError) as e:
+                bad()
+            assert e.value.status == pg.PG_ERR_INVALID_ARG
+    finally:
+        s.close()
