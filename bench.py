@@ -636,6 +636,114 @@ def batched_small(cfg, st, args):
 FP64_LANES_PER_CLK_PER_SM = 64
 
 
+def run_accel(args):
+    """--accel: the NEXT-4 variant kernels at the config's grid (default config 5): pg_acceleration (a_r, a_phi of the
+    density last set: one forward row pass, then per component one complex column pass cols_cplx_kernel and one inverse
+    row pass) and pg_potential under PG_SOFT_SOURCE (complex spectrum, one component).  Same protocol as the main line:
+    resident buffers rotated beyond L2, median of REPEATS repeats of the K-step region, parity gate against
+    oracle/polar_oracle_ext.c on seeded rings.  Algorithmic bytes per acceleration call (cells N = n_r n_phi, spectrum
+    S = 16 n_r (n_phi/2 + 1) bytes): row forward 8 N + S; per component the column pass reads S, reads the complex kernel
+    spectrum 2 S and writes S, the inverse row pass reads S and writes 8 N  ->  24 N + 11 S."""
+    import torch
+    import oracle
+    from paper_2409_02294_b200 import binding as pg, build as pg_build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if not os.path.exists(pg.LIB_PATH):
+        pg_build.build()
+    cfg = args.config
+    c = CONFIGS[cfg]
+    st = torch.cuda.Stream()
+    solver = pg.Solver(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, device=0, cuda_stream=st.cuda_stream)
+    h = solver.h
+    r, phi, _ = solver.grid()
+    field_bytes = 8 * c.n_r * c.n_phi
+    R = int(min(32, max(4, -(-4 * L2_BYTES // (3 * field_bytes)))))
+    base = [make_sigma(cfg, r, phi, b) for b in range(min(R, 4))]
+    d_sig = [torch.from_numpy(np.roll(base[k % len(base)], 97 * (k // len(base)), axis=1)).cuda() for k in range(R)]
+    d_ar = [torch.empty_like(d_sig[0]) for _ in range(R)]
+    d_ap = [torch.empty_like(d_sig[0]) for _ in range(R)]
+    torch.cuda.synchronize()
+    peak, peak_src = load_peaks()
+    spec = 16.0 * c.n_r * (c.n_phi // 2 + 1)
+    out = {}
+
+    def timed(step, steps):
+        for k in range(max(3, args.warmup)):
+            step(k)
+        pg.pg_synchronize(h)
+        rep = []
+        for _ in range(REPEATS):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(st)
+            for k in range(steps):
+                step(k)
+            e1.record(st)
+            torch.cuda.synchronize()
+            rep.append(e0.elapsed_time(e1) / steps)
+        return float(np.median(rep)), min(rep), max(rep)
+
+    def acc_step(k):
+        pg.pg_set_density(h, d_sig[k % R], 1, pg.PG_MEM_DEVICE)
+        pg.pg_acceleration(h, d_ar[k % R], d_ap[k % R], 1, pg.PG_MEM_DEVICE)
+
+    def phi_step(k):
+        pg.pg_set_density(h, d_sig[k % R], 1, pg.PG_MEM_DEVICE)
+        pg.pg_potential(h, d_ar[k % R], 1, pg.PG_MEM_DEVICE)
+
+    sampler = ClockSampler(0)
+    steps = max(1, args.steps)
+    rc = 0
+    rings = np.unique(np.random.default_rng(5).integers(0, c.n_r, 6 if c.n_r >= 1024 else 16)).astype(np.int32)
+    for soft, name in ((pg.PG_SOFT_SYMMETRIC, "symmetric"), (pg.PG_SOFT_SOURCE, "source")):
+        pg.pg_set_softening(h, soft)
+        ms, lo, hi = timed(acc_step, steps)
+        n0 = pg.pg_launch_count(h)
+        acc_step(0)
+        launches = pg.pg_launch_count(h) - n0
+        alg = 24.0 * c.n_r * c.n_phi + 11.0 * spec
+        gbs = alg / (ms * 1e-3) / 1e9
+        # parity: field 0 as the timed loop left it
+        ref_phi, ref_r, ref_p = oracle.ext_o1_rings(c.n_r, c.n_phi, c.r_in, c.r_out, c.eps, soft, base[0], rings)
+        g_r, g_p = d_ar[0].cpu().numpy()[rings], d_ap[0].cpu().numpy()[rings]
+        mag = np.hypot(ref_r, ref_p)
+        l2 = max(float(np.linalg.norm(g - q) / np.linalg.norm(q)) for g, q in ((g_r, ref_r), (g_p, ref_p)))
+        mx = max(float((np.abs(g - q) / mag).max()) for g, q in ((g_r, ref_r), (g_p, ref_p)))
+        ok = bool(l2 <= REL_L2 and mx <= MAX_REL)
+        rc = rc or (0 if ok else 3)
+        out[f"acceleration_{name}"] = {"ms_per_step": ms, "ms_min": lo, "ms_max": hi, "launches_per_step": launches,
+                                       "algorithmic_bytes_per_step": alg, "gbs": gbs, "frac_of_peak": gbs / peak,
+                                       "parity": {"rel_l2": l2, "max_rel_to_magnitude": mx, "rings": int(len(rings)), "ok": ok}}
+        if soft != pg.PG_SOFT_SYMMETRIC:
+            ms, lo, hi = timed(phi_step, steps)
+            alg = 16.0 * c.n_r * c.n_phi + 6.0 * spec          # rows 8 N + S; column pass S + 2 S + S; inverse rows S + 8 N
+            gbs = alg / (ms * 1e-3) / 1e9
+            got = d_ar[0].cpu().numpy()[rings]
+            l2 = float(np.linalg.norm(got - ref_phi) / np.linalg.norm(ref_phi)); mx = float(np.abs(got / ref_phi - 1).max())
+            ok = bool(l2 <= REL_L2 and mx <= MAX_REL)
+            rc = rc or (0 if ok else 3)
+            out[f"potential_{name}"] = {"ms_per_step": ms, "ms_min": lo, "ms_max": hi, "algorithmic_bytes_per_step": alg, "gbs": gbs,
+                                        "frac_of_peak": gbs / peak, "parity": {"rel_l2": l2, "max_rel": mx, "rings": int(len(rings)), "ok": ok}}
+    clocks = sampler.stop()
+    a = out["acceleration_source"]
+    line = {"metric": "acceleration solves/sec (fp64 FFT convolution, a_r and a_phi of one field; row NEXT-4)", "value": 1e3 / a["ms_per_step"],
+            "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": max(3, args.warmup), "ms_per_step": a["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg) + " -- pg_acceleration, PG_SOFT_SOURCE (equal to -grad Phi)", "n_r": c.n_r, "n_phi": c.n_phi,
+                       "l2": f"inputs larger than L2: steps rotate over {R} (Sigma, a_r, a_phi) buffer triples"},
+            "parity": a["parity"],
+            "roofline": {"bound": "hbm", "kernel": "whole call (rows_fwd, 2 x cols_cplx, 2 x rows_inv)", "achieved": a["gbs"], "peak": peak,
+                         "unit": "GB/s", "frac": a["frac_of_peak"], "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_step": a["algorithmic_bytes_per_step"]},
+            "variants": out, "clocks": clocks}
+    solver.close()
+    print(json.dumps(line), flush=True)
+    if rc:
+        sys.stderr.write("bench.py: PARITY GATE FAILED in --accel\n")
+    return rc
+
+
 def run_direct(args):
     """--direct: times the on-GPU cross-check (row a5, direct_kernel: tiled all-pairs summation from the
     coordinates) on one field of the config and reports pair interactions per second.  Not the headline
@@ -1034,11 +1142,14 @@ def main():
     ap.add_argument("--nested-link", default="put", choices=["put", "sendrecv"],
                     help="--nested under torchrun: one-sided puts into the neighbours' inboxes (default) or NCCL send / recv of the messages")
     ap.add_argument("--no-fused", action="store_true", help="small grids: force the three-kernel path (PG_OPT_FUSED = 0)")
+    ap.add_argument("--accel", action="store_true", help="time the NEXT-4 variant kernels (pg_acceleration, complex-spectrum potential) at --config")
     ap.add_argument("--direct", action="store_true", help="time the direct-summation cross-check kernel (a5) instead")
     ap.add_argument("--cart", type=int, default=0, choices=[0, 32, 64, 128, 256],
                     help="time the 3-D Cartesian mesh path (row NEXT-2) on an N^3 mesh instead")
     ap.add_argument("--staging", action="store_true", help="time row a6 alone: pinned vs pageable staging of a 128^3 array (PAPER.md:119)")
     args = ap.parse_args()
+    if args.accel:
+        return run_accel(args)
     if args.direct:
         return run_direct(args)
     if args.staging:
